@@ -1,0 +1,203 @@
+/* rchfsi.h -- C ABI of the B200-native R-ChFSI filter library.
+ *
+ * Method: "Residual-based Chebyshev filtered subspace iteration for Hermitian
+ * eigenvalue problems tolerant to inexact matrix-vector products" (arxiv 2503.22652).
+ * Citations are PAPER.md:LINE of the paper text this library was written from.
+ *
+ * Notation (SURVEY.md notation warning): the problem is
+ * A u = lambda B u with A Hermitian (real symmetric here), B SPD, m = matrix dimension,
+ * n_wanted = number of wanted lowest eigenpairs, N = block width (>= n_wanted),
+ * p = Chebyshev degree.  D^-1 is a cheap diagonal approximation of B^-1 (PAPER.md:164,
+ * 325) used ONLY inside the filter recurrence.
+ *
+ * Conventions
+ *  - Every function returns an rchfsi_status; nothing throws across the ABI.
+ *    rchfsi_last_error(handle) returns a static/handle-owned message for the last failure.
+ *  - Pointers documented "device" are CUDA device pointers on the current device and are
+ *    OWNED BY THE CALLER.  The library BORROWS the operator arrays and dinv_diag for the
+ *    lifetime of the handle and X / ritz / G for the duration of the call.  Pointers
+ *    documented "host" are ordinary host pointers.
+ *  - Blocks of vectors are row-major [m][N] with the N columns contiguous (one row of N
+ *    values per matrix row), FP64, 16-byte aligned.
+ *  - All device work is enqueued on the cudaStream_t given at create time (passed as
+ *    void*, NULL = the legacy default stream).  rchfsi_filter and rchfsi_rayleigh_ritz are
+ *    asynchronous with respect to the host; rchfsi_solve and the *_host entry points
+ *    synchronise the stream before returning.
+ *  - The library allocates its own device workspace (recurrence blocks, low-precision
+ *    operator copies, Rayleigh-Ritz temporaries) with cudaMalloc, lazily, and frees it in
+ *    rchfsi_destroy.  rchfsi_workspace_bytes reports the worst case up front.
+ *  - There is no CPU fallback: without a CUDA device every compute entry point returns
+ *    RCHFSI_ECUDA.
+ */
+#ifndef RCHFSI_H
+#define RCHFSI_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rchfsi_ctx *rchfsi_handle;
+
+typedef enum {
+  RCHFSI_OK = 0,
+  RCHFSI_EINVAL = 1,         /* bad argument; outputs untouched */
+  RCHFSI_ENOMEM = 2,         /* cudaMalloc / malloc failed */
+  RCHFSI_ECUDA = 3,          /* CUDA / cuBLAS / cuSOLVER runtime error, or no device */
+  RCHFSI_ENOTCONVERGED = 4,  /* rchfsi_solve hit max_iter; outputs hold the last iterate */
+  RCHFSI_EBREAKDOWN = 5      /* Rayleigh-Ritz Gram matrix Y^T B Y not numerically SPD */
+} rchfsi_status;
+
+typedef enum { RCHFSI_OP_DENSE = 0, RCHFSI_OP_CSR = 1, RCHFSI_OP_FE = 2 } rchfsi_opkind;
+
+/* Precision of the operator apply A (x) V inside the filter ("the
+ * computation of A D^-1 R_Y is done using FP32 arithmetic", TF32 compute mode, BF16).
+ * FP64: exact products (parity mode).  FP32: FP32 operands, FP32 FMA on the ALUs.
+ * TF32 / BF16: tensor-core operands, FP32 accumulate (dense and FE operators; a CSR
+ * operator treats TF32 as FP32 and BF16 as BF16-stored block with FP32 FMA). */
+typedef enum { RCHFSI_FP64 = 0, RCHFSI_FP32 = 1, RCHFSI_TF32 = 2, RCHFSI_BF16 = 3 } rchfsi_prec;
+
+/* RCHFSI_METHOD_CHFSI: Algorithm 2 with H = D^-1 (A (x) .)  (eq. (7) at 170).
+ * RCHFSI_METHOD_RCHFSI: Algorithm 3, the recurrence on residuals. */
+typedef enum { RCHFSI_METHOD_CHFSI = 0, RCHFSI_METHOD_RCHFSI = 1 } rchfsi_method;
+
+/* A linear operator on R^m.  All arrays are device pointers, FP64 master copies.
+ *  DENSE: `dense` row-major m x m with leading dimension lda (>= m), symmetric.
+ *  CSR  : rowptr[m+1] (int64), colind[nnz] (int32, any order within a row), vals[nnz].
+ *  FE   : A V = sum_c P_c^T A_c P_c V (Remark 4.1): conn[n_cells][n_loc]
+ *         holds the global row of each local node (distinct within a cell);
+ *         cell_mats is [n_cells][n_loc][n_loc], or ONE [n_loc][n_loc] matrix shared by
+ *         every cell when cell_shared != 0.  Every cell matrix must be symmetric (it is
+ *         the element matrix of a symmetric form; A is Hermitian): the
+ *         kernels read A_c[b][a] for A_c[a][b].  rchfsi_create verifies this.
+ *         cell_mats_f32, if non-NULL, is the same array in FP32 and may be given INSTEAD
+ *         of cell_mats (cell_mats == NULL) when the FP64 copy does not fit (config 5:
+ *         13 GB); it is then also what the FP64 Rayleigh-Ritz path reads (widened). */
+typedef struct {
+  int32_t kind;               /* rchfsi_opkind */
+  int64_t m;
+  const double *dense;
+  int64_t lda;
+  const int64_t *rowptr;
+  const int32_t *colind;
+  const double *vals;
+  int64_t nnz;
+  int64_t n_cells;
+  int32_t n_loc;
+  int32_t cell_shared;
+  const double *cell_mats;
+  const float *cell_mats_f32;
+  const int32_t *conn;
+} rchfsi_operator;
+
+typedef struct {
+  int32_t apply_prec;         /* rchfsi_prec of the operator apply inside the filter */
+  int32_t store_prec;         /* RCHFSI_FP64 or RCHFSI_FP32: storage of R_X, R_Y and of the
+                                 filter's copy of G (PAPER.md:341 stores them in FP32) */
+  int32_t normalize_columns_before_rr; /* scale columns of Y_p to unit 2-norm before the
+                                 Gram matrices (reading S6); default 1 */
+  int32_t adaptive_bounds;    /* rchfsi_solve: after each Rayleigh-Ritz set lam_T to the
+                                 largest and lam_min to the smallest Ritz value (S7) */
+  double noise_eps;           /* > 0: debug hook, per-matvec column-scaled Gaussian error
+                                 T_j += eps ||T_j|| g_j/||g_j|| inside the filter only
+                                 (BASELINE.json configs[0]; reading S11) */
+  uint64_t noise_seed;
+  int32_t use_cuda_graph;     /* capture the p-1 recurrence steps in a CUDA graph */
+  int32_t reserved;
+} rchfsi_options;
+
+/* Fill `opt` with the defaults: apply FP64, store FP64, normalize 1, everything else 0. */
+void rchfsi_default_options(rchfsi_options *opt);
+
+/* Create a solver context for A x = lambda B x.
+ *  A          operator (borrowed).
+ *  B          operator or NULL for B = I (the standard problem).
+ *  dinv_diag  device, length m: diagonal of D^-1 ~ B^-1; NULL => I.
+ *  block_N    block width N (1 <= N <= m).
+ *  opt        NULL => defaults.
+ *  cuda_stream cudaStream_t as void*.
+ * Errors: EINVAL (null/ill-sized arguments, unknown kind/precision, non-symmetric FE cell
+ * matrices), ECUDA (no device), ENOMEM. */
+rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A,
+                            const rchfsi_operator *B, const double *dinv_diag,
+                            int32_t block_N, const rchfsi_options *opt, void *cuda_stream);
+
+rchfsi_status rchfsi_destroy(rchfsi_handle h);
+
+/* Message for the most recent failure on this handle ("" if none); NULL handle => the
+ * message of the last failed rchfsi_create in this thread. */
+const char *rchfsi_last_error(rchfsi_handle h);
+
+/* Worst-case device bytes the handle will allocate for the given problem (recurrence
+ * blocks + low-precision operator copy + Rayleigh-Ritz temporaries). */
+size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B,
+                              int32_t block_N, const rchfsi_options *opt);
+
+/* The Chebyshev filter (the hot path).
+ *  method RCHFSI (Algorithm 3):
+ *     R_X = 0, R_Y = (sigma_1/e) G, Lambda_X = I, Lambda_Y = (sigma_1/e)(Lambda - c I);
+ *     for k = 2..p:  R_X <- a A (x) (D^-1 R_Y) + b R_Y + c' R_X + a G Lambda_Y,
+ *                    Lambda_X <- a Lambda_Y Lambda + b Lambda_Y + c' Lambda_X, swap;
+ *     X <- D^-1 R_Y + X Lambda_Y,
+ *     with e, c, sigma_1, sigma_{k+1} = 1/(2/sigma_1 - sigma_k), a = 2 sigma_{k+1}/e,
+ *     b = -a c, c' = -sigma_k sigma_{k+1}.
+ *  method CHFSI (Algorithm 2, PAPER.md:78-86 with eq. (7) at 170):
+ *     Y = (sigma_1/e)(D^-1 A (x) X - c X); for k = 2..p: X <- a D^-1 A (x) Y + b Y + c' X, swap.
+ *  X      device [m][N] FP64, in: X^(i); out: the filtered block Y_p (overwritten).
+ *  ritz   device [N] FP64: diagonal of Lambda^(i) (RCHFSI only; ignored for CHFSI).
+ *  G      device [m][N] FP64: A X - B X Lambda computed with the exact
+ *         operators; NULL => computed here in FP64 from A, B, X, ritz (RCHFSI only).
+ *  degree p >= 1; lam_min < lam_T < lam_max (a_low <= lambda_1, [a,b] = [lam_T, lam_max]).
+ * Asynchronous.  Errors: EINVAL (bad handle / pointers / degree / bounds), ECUDA, ENOMEM. */
+rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const double *ritz,
+                            const double *G, int32_t degree, double lam_min, double lam_T,
+                            double lam_max);
+
+/* Same call with HOST buffers: copies X, ritz (and G if non-NULL) to device scratch,
+ * runs rchfsi_filter, copies Y_p back into X_host, synchronises. */
+rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host,
+                                 const double *ritz_host, const double *G_host,
+                                 int32_t degree, double lam_min, double lam_T, double lam_max);
+
+/* Rayleigh-Ritz on a non-orthogonal basis, all in FP64 with the
+ * exact operators: H_a = Y^T A Y, H_b = Y^T B Y, solve H_a E = H_b E Lambda with
+ * E^T H_b E = I and ascending eigenvalues, X = Y E.
+ *  Y_in_X_out  device [m][N]: in the basis Y (columns scaled to unit 2-norm first when
+ *              normalize_columns_before_rr), out the B-orthonormal Ritz vectors X.
+ *  ritz_out    device [N]: Ritz values, ascending.
+ *  G_out       device [m][N] or NULL: A X - B X diag(ritz) (the input of Algorithm 3).
+ *  resnorm_out device [N] or NULL: r_j = ||A x_j - ritz_j B x_j||_2.
+ * Asynchronous except for one host read of the cuSOLVER status (EBREAKDOWN). */
+rchfsi_status rchfsi_rayleigh_ritz(rchfsi_handle h, double *Y_in_X_out, double *ritz_out,
+                                   double *G_out, double *resnorm_out);
+
+/* Algorithm 1, do-while reading: one Rayleigh-Ritz on the initial guess,
+ * then repeat { filter; Rayleigh-Ritz; residual test on the n_wanted lowest pairs }.
+ *  X            device [m][N]: in the initial guess, out B-orthonormal Ritz vectors.
+ *  evals_out    HOST [N]; resnorm_out HOST [N]; iters_out HOST (outer iterations done).
+ *  history_out  HOST [max_iter] or NULL: max wanted residual after each iteration.
+ * Returns OK when max_{j<n_wanted} r_j < tol, ENOTCONVERGED otherwise. */
+rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n_wanted,
+                           int32_t degree, double lam_min, double lam_T, double lam_max,
+                           double tol, int32_t max_iter, double *evals_out,
+                           double *resnorm_out, int32_t *iters_out, double *history_out);
+
+/* Exact FP64 operator apply, exposed for tests and residual certification:
+ * which = 0: out = A V, which = 1: out = B V (B = I copies).  V, out device [m][N]. */
+rchfsi_status rchfsi_apply(rchfsi_handle h, int32_t which, const double *V, double *out);
+
+/* Instrumentation: number of kernels this handle has launched since creation, and the
+ * CUDA-event time (ms) of the recurrence-step launches of the last rchfsi_filter call
+ * (steps_out = number of step launches timed; needs a stream synchronise, which it does). */
+int64_t rchfsi_launch_count(rchfsi_handle h);
+rchfsi_status rchfsi_last_filter_step_ms(rchfsi_handle h, float *ms_total_out, int32_t *steps_out);
+
+/* Library / build identification, e.g. "rchfsi 0.1 sm_100a". */
+const char *rchfsi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RCHFSI_H */

@@ -1,0 +1,261 @@
+"""Thin ctypes binding of librchfsi.so (include/rchfsi.h): argument marshalling only.
+
+Every step of the filter path runs in the library's CUDA kernels.  PyTorch is used for device
+memory (torch tensors own the buffers whose data_ptr() crosses the C ABI) and for the stream.
+There is no CPU fallback: a missing or unloadable library raises at import / first use.
+"""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "librchfsi.so")
+
+OK, EINVAL, ENOMEM, ECUDA, ENOTCONVERGED, EBREAKDOWN = range(6)
+OP_DENSE, OP_CSR, OP_FE = 0, 1, 2
+FP64, FP32, TF32, BF16 = 0, 1, 2, 3
+METHOD_CHFSI, METHOD_RCHFSI = 0, 1
+PREC = {"fp64": FP64, "fp32": FP32, "tf32": TF32, "bf16": BF16}
+STATUS_NAME = {0: "OK", 1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "ENOTCONVERGED", 5: "EBREAKDOWN"}
+
+
+class RchfsiOperator(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("m", C.c_int64), ("dense", C.c_void_p), ("lda", C.c_int64),
+                ("rowptr", C.c_void_p), ("colind", C.c_void_p), ("vals", C.c_void_p), ("nnz", C.c_int64),
+                ("n_cells", C.c_int64), ("n_loc", C.c_int32), ("cell_shared", C.c_int32),
+                ("cell_mats", C.c_void_p), ("cell_mats_f32", C.c_void_p), ("conn", C.c_void_p)]
+
+
+class RchfsiOptions(C.Structure):
+    _fields_ = [("apply_prec", C.c_int32), ("store_prec", C.c_int32),
+                ("normalize_columns_before_rr", C.c_int32), ("adaptive_bounds", C.c_int32),
+                ("noise_eps", C.c_double), ("noise_seed", C.c_uint64),
+                ("use_cuda_graph", C.c_int32), ("reserved", C.c_int32)]
+
+
+# every symbol include/rchfsi.h declares: name -> (restype, argtypes)
+SYMBOLS = {
+    "rchfsi_version": (C.c_char_p, []),
+    "rchfsi_default_options": (None, [C.POINTER(RchfsiOptions)]),
+    "rchfsi_create": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(RchfsiOperator), C.POINTER(RchfsiOperator),
+                                C.c_void_p, C.c_int32, C.POINTER(RchfsiOptions), C.c_void_p]),
+    "rchfsi_destroy": (C.c_int, [C.c_void_p]),
+    "rchfsi_last_error": (C.c_char_p, [C.c_void_p]),
+    "rchfsi_workspace_bytes": (C.c_size_t, [C.POINTER(RchfsiOperator), C.POINTER(RchfsiOperator), C.c_int32,
+                                            C.POINTER(RchfsiOptions)]),
+    "rchfsi_filter": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                C.c_double, C.c_double, C.c_double]),
+    "rchfsi_filter_host": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                     C.c_double, C.c_double, C.c_double]),
+    "rchfsi_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rchfsi_solve": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
+                               C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p,
+                               C.POINTER(C.c_int32), C.c_void_p]),
+    "rchfsi_apply": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
+    "rchfsi_launch_count": (C.c_int64, [C.c_void_p]),
+    "rchfsi_last_filter_step_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]),
+}
+
+_lib = None
+
+
+def load_library():
+    """dlopen librchfsi.so and type every exported symbol.  Raises if the library is missing
+    (build it with `python -m paper_2503_22652_b200.build`): there is no fallback path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("librchfsi.so is not built (%s); run python -m paper_2503_22652_b200.build"
+                           % LIB_PATH)
+    lib = C.CDLL(LIB_PATH, mode=C.RTLD_GLOBAL)
+    for name, (res, args) in SYMBOLS.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+class RchfsiError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS_NAME.get(status, status), message))
+        self.status = status
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _check_dev(t, dtype, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous CUDA tensor of %s" % (name, dtype))
+    return t
+
+
+def make_operator(spec, keep):
+    """spec: dict(kind='dense', A=tensor) | dict(kind='csr', rowptr, colind, vals) |
+    dict(kind='fe', conn, cell_mats=None, cell_mats_f32=None, shared=False, m=...)  (CUDA tensors).
+    `keep` collects the tensors so they outlive the handle."""
+    import torch
+    op = RchfsiOperator()
+    kind = spec["kind"]
+    if kind == "dense":
+        A = _check_dev(spec["A"], torch.float64, "A")
+        op.kind, op.m, op.dense, op.lda = OP_DENSE, A.shape[0], A.data_ptr(), A.shape[1]
+        keep.append(A)
+    elif kind == "csr":
+        rp = _check_dev(spec["rowptr"], torch.int64, "rowptr")
+        ci = _check_dev(spec["colind"], torch.int32, "colind")
+        va = _check_dev(spec["vals"], torch.float64, "vals")
+        op.kind, op.m = OP_CSR, rp.numel() - 1
+        op.rowptr, op.colind, op.vals, op.nnz = rp.data_ptr(), ci.data_ptr(), va.data_ptr(), va.numel()
+        keep += [rp, ci, va]
+    elif kind == "fe":
+        conn = _check_dev(spec["conn"], torch.int32, "conn")
+        op.kind, op.m = OP_FE, int(spec["m"])
+        op.n_cells, op.n_loc = conn.shape[0], conn.shape[1]
+        op.cell_shared = 1 if spec.get("shared") else 0
+        op.conn = conn.data_ptr()
+        keep.append(conn)
+        if spec.get("cell_mats") is not None:
+            cm = _check_dev(spec["cell_mats"], torch.float64, "cell_mats")
+            op.cell_mats = cm.data_ptr()
+            keep.append(cm)
+        if spec.get("cell_mats_f32") is not None:
+            cf = _check_dev(spec["cell_mats_f32"], torch.float32, "cell_mats_f32")
+            op.cell_mats_f32 = cf.data_ptr()
+            keep.append(cf)
+    else:
+        raise ValueError(kind)
+    return op
+
+
+class Rchfsi:
+    """Handle wrapper.  Method names mirror the C entry points (rchfsi_filter -> .filter, ...)."""
+
+    def __init__(self, A, B=None, dinv=None, block_N=1, apply_prec="fp64", store_prec="fp64",
+                 normalize_columns_before_rr=True, adaptive_bounds=False, noise_eps=0.0, noise_seed=0,
+                 use_cuda_graph=False, stream=None):
+        import torch
+        self.lib = load_library()
+        self._keep = []
+        self.opA = make_operator(A, self._keep)
+        self.opB = make_operator(B, self._keep) if B is not None else None
+        if dinv is not None:
+            self._keep.append(_check_dev(dinv, torch.float64, "dinv"))
+        opt = RchfsiOptions()
+        self.lib.rchfsi_default_options(C.byref(opt))
+        opt.apply_prec = PREC[apply_prec] if isinstance(apply_prec, str) else apply_prec
+        opt.store_prec = PREC[store_prec] if isinstance(store_prec, str) else store_prec
+        opt.normalize_columns_before_rr = int(normalize_columns_before_rr)
+        opt.adaptive_bounds = int(adaptive_bounds)
+        opt.noise_eps = float(noise_eps)
+        opt.noise_seed = int(noise_seed)
+        opt.use_cuda_graph = int(use_cuda_graph)
+        self.opt = opt
+        self.m, self.N = int(self.opA.m), int(block_N)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        h = C.c_void_p()
+        st = self.lib.rchfsi_create(C.byref(h), C.byref(self.opA),
+                                    C.byref(self.opB) if self.opB is not None else None,
+                                    _ptr(dinv), self.N, C.byref(opt), C.c_void_p(self.stream.cuda_stream))
+        if st != OK:
+            raise RchfsiError(st, (self.lib.rchfsi_last_error(None) or b"").decode())
+        self.h = h
+
+    def _raise(self, st):
+        raise RchfsiError(st, (self.lib.rchfsi_last_error(self.h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.rchfsi_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _block(self, t, name):
+        import torch
+        _check_dev(t, torch.float64, name)
+        if tuple(t.shape) != (self.m, self.N):
+            raise ValueError("%s must have shape (%d, %d)" % (name, self.m, self.N))
+        return t
+
+    def filter(self, method, X, ritz, G, degree, lam_min, lam_T, lam_max):
+        """rchfsi_filter: X [m][N] CUDA float64 is overwritten by the filtered block Y_p."""
+        import torch
+        self._block(X, "X")
+        if G is not None:
+            self._block(G, "G")
+        if ritz is not None:
+            _check_dev(ritz, torch.float64, "ritz")
+        st = self.lib.rchfsi_filter(self.h, method, _ptr(X), _ptr(ritz), _ptr(G), degree, lam_min, lam_T, lam_max)
+        if st != OK:
+            self._raise(st)
+        return X
+
+    def filter_host(self, method, X_host, ritz_host, G_host, degree, lam_min, lam_T, lam_max):
+        """rchfsi_filter_host: numpy / CPU-tensor buffers (float64, C-contiguous); X_host is
+        overwritten with Y_p.  Host<->device copies happen inside the call."""
+        def hp(a):
+            if a is None:
+                return C.c_void_p(0)
+            return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+        st = self.lib.rchfsi_filter_host(self.h, method, hp(X_host), hp(ritz_host), hp(G_host), degree,
+                                         lam_min, lam_T, lam_max)
+        if st != OK:
+            self._raise(st)
+        return X_host
+
+    def rayleigh_ritz(self, Y, want_G=True):
+        """rchfsi_rayleigh_ritz: returns (ritz, X (= Y overwritten), G or None, resnorm)."""
+        import torch
+        self._block(Y, "Y")
+        ritz = torch.empty(self.N, dtype=torch.float64, device=Y.device)
+        res = torch.empty(self.N, dtype=torch.float64, device=Y.device)
+        G = torch.empty_like(Y) if want_G else None
+        st = self.lib.rchfsi_rayleigh_ritz(self.h, _ptr(Y), _ptr(ritz), _ptr(G), _ptr(res))
+        if st != OK:
+            self._raise(st)
+        return ritz, Y, G, res
+
+    def solve(self, method, X, n_wanted, degree, lam_min, lam_T, lam_max, tol=1e-8, max_iter=50,
+              raise_on_not_converged=False):
+        """rchfsi_solve: returns dict(evals, resnorm, iters, history, converged); X overwritten."""
+        import numpy as np
+        self._block(X, "X")
+        evals = np.empty(self.N)
+        res = np.empty(self.N)
+        hist = np.full(max_iter, np.nan)
+        iters = C.c_int32(0)
+        st = self.lib.rchfsi_solve(self.h, method, _ptr(X), n_wanted, degree, lam_min, lam_T, lam_max, tol,
+                                   max_iter, C.c_void_p(evals.ctypes.data), C.c_void_p(res.ctypes.data),
+                                   C.byref(iters), C.c_void_p(hist.ctypes.data))
+        if st not in (OK, ENOTCONVERGED) or (st == ENOTCONVERGED and raise_on_not_converged):
+            self._raise(st)
+        return dict(evals=evals, resnorm=res, iters=iters.value, history=hist[:iters.value],
+                    converged=(st == OK))
+
+    def apply(self, which, V):
+        """rchfsi_apply: exact FP64 A V (which=0) or B V (which=1)."""
+        import torch
+        self._block(V, "V")
+        out = torch.empty_like(V)
+        st = self.lib.rchfsi_apply(self.h, which, _ptr(V), _ptr(out))
+        if st != OK:
+            self._raise(st)
+        return out
+
+    def launch_count(self):
+        return int(self.lib.rchfsi_launch_count(self.h))
+
+    def last_filter_step_ms(self):
+        ms, n = C.c_float(0), C.c_int32(0)
+        st = self.lib.rchfsi_last_filter_step_ms(self.h, C.byref(ms), C.byref(n))
+        if st != OK:
+            self._raise(st)
+        return ms.value, n.value

@@ -1,0 +1,198 @@
+// Internal definitions shared by the translation units of librchfsi.so.
+// Nothing here is visible across the C ABI (include/rchfsi.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <cublas_v2.h>
+#include <cusolverDn.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "rchfsi.h"
+
+namespace rchfsi {
+
+// One recurrence step's scalars, Alg. 3 loop body:
+//   out = a * T * (dinv_out ? dinv[i] : 1) + b * RY + cp * RX + (has_G ? a * G * LY[j] : 0)
+struct StepCoef {
+  double a, b, cp;
+};
+
+// Low-precision device copy of an operator for the tensor-core paths.
+struct LowpCopy {
+  int prec = -1;          // RCHFSI_TF32 / RCHFSI_BF16 / RCHFSI_FP32
+  bool folded = false;    // columns pre-scaled by dinv (A * diag(dinv))
+  void *data = nullptr;   // dense: [m_pad][k_pad]; FE: [n_cells][a_pad][k_pad]
+  int64_t ld = 0;         // padded K extent (elements)
+  int64_t rows_pad = 0;   // padded row extent per matrix
+  size_t bytes = 0;
+};
+
+struct DeviceOperator {
+  rchfsi_operator d{};    // caller's descriptor (device pointers, borrowed)
+  bool present = false;
+};
+
+// FE colouring (host-built at create): cells of one colour share no node.
+struct FeColoring {
+  int n_colors = 0;
+  std::vector<int64_t> color_begin;   // [n_colors + 1] into cell_order
+  int32_t *cell_order = nullptr;      // device [n_cells], cells grouped by colour
+  uint8_t *flags = nullptr;           // device [n_cells][n_loc]: bit0 first toucher, bit1 last toucher
+};
+
+}  // namespace rchfsi
+
+struct rchfsi_ctx {
+  rchfsi::DeviceOperator A, B;
+  const double *dinv = nullptr;
+  int64_t m = 0;
+  int32_t N = 0;
+  rchfsi_options opt{};
+  cudaStream_t stream = nullptr;
+  cublasHandle_t cublas = nullptr;
+  cusolverDnHandle_t cusolver = nullptr;
+  std::string err;
+  int64_t launches = 0;
+
+  // filter workspace (storage precision), lazily allocated
+  void *RX = nullptr, *RY = nullptr;      // [m][N] store_prec
+  void *Gs = nullptr;                     // [m][N] store_prec copy of G (store FP32 only)
+  void *Wa = nullptr, *Wb = nullptr;      // operand-precision shadows of R_Y (when needed)
+  void *T = nullptr;                      // [m][N] operator output for the unfused paths
+  double *Gtmp = nullptr;                 // [m][N] FP64 when G == NULL is computed here
+  double *lam_table = nullptr;            // [(p_max+1)][N]
+  int32_t lam_table_p = 0;
+  double *colnorm = nullptr;              // [2][N]
+  std::vector<rchfsi::LowpCopy> lowp;
+  rchfsi::FeColoring coloring;
+
+  // Rayleigh-Ritz workspace
+  double *rr1 = nullptr, *rr2 = nullptr, *rr3 = nullptr;   // [m][N] FP64
+  double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
+  double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
+  double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
+
+  // host-buffer entry point scratch
+  double *hX = nullptr, *hG = nullptr, *hritz = nullptr;
+
+  // instrumentation
+  cudaEvent_t ev_step0 = nullptr, ev_step1 = nullptr;
+  int32_t last_steps = 0;
+
+  std::vector<void *> owned;   // everything cudaMalloc'ed by this handle
+};
+
+namespace rchfsi {
+
+#define RCHFSI_CUDA_CHECK(h, expr)                                                        \
+  do {                                                                                    \
+    cudaError_t _e = (expr);                                                              \
+    if (_e != cudaSuccess) {                                                              \
+      (h)->err = std::string(#expr) + ": " + cudaGetErrorString(_e);                      \
+      return (_e == cudaErrorMemoryAllocation) ? RCHFSI_ENOMEM : RCHFSI_ECUDA;            \
+    }                                                                                     \
+  } while (0)
+
+#define RCHFSI_TRY(expr)                        \
+  do {                                          \
+    rchfsi_status _s = (expr);                  \
+    if (_s != RCHFSI_OK) return _s;             \
+  } while (0)
+
+rchfsi_status dev_alloc(rchfsi_ctx *h, void **p, size_t bytes);
+static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+#define LAUNCH_CHECK(h)                                                                   \
+  do {                                                                                    \
+    (h)->launches++;                                                                      \
+    cudaError_t _e = cudaGetLastError();                                                  \
+    if (_e != cudaSuccess) {                                                              \
+      (h)->err = std::string("kernel launch: ") + cudaGetErrorString(_e) + " at " +      \
+                 __FILE__ + ":" + std::to_string(__LINE__);                               \
+      return RCHFSI_ECUDA;                                                                \
+    }                                                                                     \
+  } while (0)
+
+inline size_t prec_bytes(int prec) {
+  return prec == RCHFSI_FP64 ? 8 : (prec == RCHFSI_BF16 ? 2 : 4);
+}
+
+// ---- kernels_simt.cu ------------------------------------------------------------------
+// T = A * (dinv_in ? diag(dinv) : I) * W for W, T of element type TW / TO in {double, float}.
+// For FE the output is accumulated with atomics into a zeroed T.
+template <typename TC>
+rchfsi_status op_apply_simt(rchfsi_ctx *h, const rchfsi_operator &op, const double *dinv_in,
+                            const TC *W, TC *T, int32_t N);
+
+// Lambda_k table, k = 0..p (eq. (12)): table[k][j].
+rchfsi_status lambda_table(rchfsi_ctx *h, const double *ritz, int32_t N, int32_t p, double e,
+                           double c, double sigma1, double *table);
+
+// Element-wise pieces of Alg. 2 / Alg. 3 (storage type S, operand shadow type O, T type TT).
+struct StepArgs {
+  StepCoef k;
+  const void *T;        // operator output
+  const void *RY;       // storage
+  void *RX;             // storage, in: R_X (old), out: R_X (new)
+  const void *G;        // storage or NULL
+  const double *LY;     // Lambda_Y row of the table (device) or NULL
+  const double *dinv_out;  // CHFSI: row scaling of T, else NULL
+  void *Wnext;          // operand-precision shadow of the new block, or NULL
+  int64_t m;
+  int32_t N;
+};
+rchfsi_status step_elementwise(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_prec,
+                               const StepArgs &a);
+// dst(store) = alpha * src(FP64) (+ shadow), used for R_Y = (sigma_1/e) G and G copies
+rchfsi_status scale_convert(rchfsi_ctx *h, int store_prec, int shadow_prec, double alpha,
+                            const double *src, void *dst, void *shadow, int64_t m, int32_t N);
+// CHFSI first step: Y = alpha * (dinv * T - c X)
+rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_prec, double alpha,
+                          double c, const void *T, const double *dinv, const double *X, void *Y,
+                          void *shadow, int64_t m, int32_t N);
+// RCHFSI finish: X = dinv * RY + X * LY (PAPER.md:263 last line); CHFSI finish: X = RY
+rchfsi_status finish_block(rchfsi_ctx *h, int store_prec, const void *RY, const double *dinv,
+                           const double *LY, double *X, int64_t m, int32_t N);
+// FP64 -> operand precision shadow of X (CHFSI start)
+rchfsi_status convert_block(rchfsi_ctx *h, int dst_prec, const double *src, void *dst, int64_t m,
+                            int32_t N);
+// column 2-norms (sum of squares accumulated in FP64 with atomics into a zeroed array)
+rchfsi_status column_sumsq(rchfsi_ctx *h, int prec, const void *V, int64_t m, int32_t N,
+                           double *sumsq);
+rchfsi_status scale_columns_inv_norm(rchfsi_ctx *h, double *V, int64_t m, int32_t N,
+                                     const double *sumsq);
+// T_j += eps ||T_j|| g_j / ||g_j||, g = counter-based Gaussian (S11)
+rchfsi_status add_column_noise(rchfsi_ctx *h, int t_prec, void *T, int64_t m, int32_t N, double eps,
+                               uint64_t seed, uint64_t apply_index, double *scratch2N);
+// G = AX - BX diag(ritz), res_j = ||G_j||
+rchfsi_status residual_block(rchfsi_ctx *h, const double *AX, const double *BX, const double *ritz,
+                             double *G, double *res, int64_t m, int32_t N);
+rchfsi_status symmetrize(rchfsi_ctx *h, double *H, int32_t N);
+rchfsi_status fe_check_symmetric(rchfsi_ctx *h, const rchfsi_operator &op, double *max_asym_host);
+
+// ---- fused paths (return RCHFSI_EINVAL if the configuration is not supported so the caller
+// can fall back to the unfused sequence) -------------------------------------------------
+struct FusedStep {
+  StepCoef k;
+  const void *W;        // operand block (shadow or R_Y itself)
+  const void *RY;
+  void *RX;
+  const void *G;
+  const double *LY;
+  void *Wnext;
+  int apply_prec, store_prec;
+  bool chfsi;           // dinv applied to the output rows instead of the input
+};
+bool csr_fused_supported(const rchfsi_ctx *h);
+rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s);
+bool dense_tc_supported(const rchfsi_ctx *h);
+rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s);
+bool fe_tc_supported(const rchfsi_ctx *h);
+rchfsi_status fe_tc_step(rchfsi_ctx *h, const FusedStep &s);
+
+// ---- rr.cu -----------------------------------------------------------------------------
+rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, double *G_out,
+                                 double *res_out);
+
+}  // namespace rchfsi

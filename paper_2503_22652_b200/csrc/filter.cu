@@ -1,0 +1,246 @@
+// rchfsi_filter / rchfsi_filter_host / rchfsi_solve: host control flow of Algorithm 2
+// (PAPER.md:78-86), Algorithm 3 and Algorithm 1.
+#include <cmath>
+#include "common.cuh"
+
+using namespace rchfsi;
+
+namespace {
+
+struct Plan {
+  int store;     // storage precision of R_X, R_Y, G
+  int operand;   // precision of the block the operator kernel reads
+  int tprec;     // precision of the unfused operator output T
+  bool shadow;   // operand block is a separate buffer
+  int fused;     // 0 unfused SIMT, 1 CSR fused, 2 dense tensor-core, 3 FE tensor-core
+};
+
+Plan make_plan(const rchfsi_ctx *h) {
+  Plan p{};
+  p.store = h->opt.store_prec;
+  const int ap = h->opt.apply_prec;
+  p.fused = 0;
+  if (ap == RCHFSI_FP64) {
+    p.operand = RCHFSI_FP64;
+  } else {
+    p.operand = RCHFSI_FP32;
+    if (h->opt.noise_eps <= 0) {
+      if (h->A.d.kind == RCHFSI_OP_CSR && csr_fused_supported(h)) p.fused = 1;
+      if (h->A.d.kind == RCHFSI_OP_DENSE && ap != RCHFSI_FP32 && dense_tc_supported(h)) p.fused = 2;
+      if (h->A.d.kind == RCHFSI_OP_FE && ap != RCHFSI_FP32 && fe_tc_supported(h)) p.fused = 3;
+    }
+    if (p.fused >= 2 && ap == RCHFSI_BF16) p.operand = RCHFSI_BF16;
+    if (p.fused == 1) p.operand = p.store;   // the CSR kernel reads R_Y itself, converting on the fly
+  }
+  p.tprec = (ap == RCHFSI_FP64) ? RCHFSI_FP64 : RCHFSI_FP32;
+  p.shadow = (p.operand != p.store);
+  return p;
+}
+
+rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t degree, bool need_gs) {
+  const size_t el = (size_t)h->m * h->N;
+  if (!h->RX) RCHFSI_TRY(dev_alloc(h, &h->RX, el * prec_bytes(pl.store)));
+  if (!h->RY) RCHFSI_TRY(dev_alloc(h, &h->RY, el * prec_bytes(pl.store)));
+  if (pl.shadow) {
+    if (!h->Wa) RCHFSI_TRY(dev_alloc(h, &h->Wa, el * 4));
+    if (!h->Wb) RCHFSI_TRY(dev_alloc(h, &h->Wb, el * 4));
+  }
+  if (pl.fused == 0 && !h->T) RCHFSI_TRY(dev_alloc(h, &h->T, el * prec_bytes(pl.tprec)));
+  if (need_gs && !h->Gs) RCHFSI_TRY(dev_alloc(h, &h->Gs, el * prec_bytes(pl.store)));
+  if (!h->lam_table || h->lam_table_p < degree) {
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->lam_table, sizeof(double) * (size_t)(degree + 1) * h->N));
+    h->lam_table_p = degree;
+  }
+  if (!h->colnorm) RCHFSI_TRY(dev_alloc(h, (void **)&h->colnorm, sizeof(double) * 2 * h->N));
+  return RCHFSI_OK;
+}
+
+// One operator apply + recurrence update, fused when a fused kernel exists for this plan.
+rchfsi_status do_step(rchfsi_ctx *h, const Plan &pl, bool chfsi, const StepCoef &k, const void *W,
+                      const void *RY, void *RX, const void *G, const double *LY, void *Wnext,
+                      uint64_t apply_index) {
+  if (pl.fused) {
+    FusedStep s{k, W, RY, RX, G, LY, Wnext, h->opt.apply_prec, pl.store, chfsi};
+    if (pl.fused == 1) return csr_fused_step(h, s);
+    if (pl.fused == 2) return dense_tc_step(h, s);
+    return fe_tc_step(h, s);
+  }
+  const double *dinv_in = chfsi ? nullptr : h->dinv;
+  if (pl.tprec == RCHFSI_FP64)
+    RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, dinv_in, (const double *)W, (double *)h->T, h->N));
+  else
+    RCHFSI_TRY(op_apply_simt<float>(h, h->A.d, dinv_in, (const float *)W, (float *)h->T, h->N));
+  if (h->opt.noise_eps > 0)
+    RCHFSI_TRY(add_column_noise(h, pl.tprec, h->T, h->m, h->N, h->opt.noise_eps, h->opt.noise_seed,
+                                apply_index, h->colnorm));
+  StepArgs a{k, h->T, RY, RX, G, LY, chfsi ? h->dinv : nullptr, Wnext, h->m, h->N};
+  return step_elementwise(h, pl.store, pl.tprec, pl.operand, a);
+}
+
+}  // namespace
+
+extern "C" {
+
+rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const double *ritz, const double *G,
+                            int32_t degree, double lam_min, double lam_T, double lam_max) {
+  if (!h) return RCHFSI_EINVAL;
+  if (!X || (reinterpret_cast<uintptr_t>(X) & 15u)) { h->err = "rchfsi_filter: X null or misaligned"; return RCHFSI_EINVAL; }
+  if (method != RCHFSI_METHOD_CHFSI && method != RCHFSI_METHOD_RCHFSI) { h->err = "rchfsi_filter: unknown method"; return RCHFSI_EINVAL; }
+  if (method == RCHFSI_METHOD_RCHFSI && !ritz) { h->err = "rchfsi_filter: ritz is required for R-ChFSI"; return RCHFSI_EINVAL; }
+  if (G && (reinterpret_cast<uintptr_t>(G) & 15u)) { h->err = "rchfsi_filter: G misaligned"; return RCHFSI_EINVAL; }
+  if (degree < 1) { h->err = "rchfsi_filter: degree < 1"; return RCHFSI_EINVAL; }
+  if (!(lam_min < lam_T) || !(lam_T < lam_max) || !std::isfinite(lam_min) || !std::isfinite(lam_max)) {
+    h->err = "rchfsi_filter: need lam_min < lam_T < lam_max";
+    return RCHFSI_EINVAL;
+  }
+  const bool chfsi = (method == RCHFSI_METHOD_CHFSI);
+  const Plan pl = make_plan(h);
+  const int64_t m = h->m;
+  const int32_t N = h->N;
+  const size_t el = (size_t)m * N;
+  cudaStream_t st = h->stream;
+  const bool need_gs = !chfsi && pl.store != RCHFSI_FP64;
+  RCHFSI_TRY(ensure_filter_workspace(h, pl, degree, need_gs));
+
+  // first line of Alg. 2 / Alg. 3
+  const double e = (lam_max - lam_T) / 2.0;
+  const double c = (lam_max + lam_T) / 2.0;
+  const double sigma1 = e / (lam_min - c);
+  const double gamma = 2.0 / sigma1;
+  double sigma = sigma1;
+
+  void *RX = h->RX, *RY = h->RY;
+  void *Wcur = pl.shadow ? h->Wa : nullptr, *Wnext = pl.shadow ? h->Wb : nullptr;
+  const void *Gst = nullptr;
+  uint64_t apply_index = 0;
+
+  if (!chfsi) {
+    // G = A X - B X Lambda with the exact operators (reading S5) when the caller has none
+    if (!G) {
+      if (!h->Gtmp) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gtmp, el * 8));
+      if (!h->rr1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr1, el * 8));
+      RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, X, h->rr1, N));
+      const double *BX = X;
+      if (h->B.present) {
+        RCHFSI_TRY(op_apply_simt<double>(h, h->B.d, nullptr, X, h->Gtmp, N));
+        BX = h->Gtmp;
+      }
+      RCHFSI_TRY(residual_block(h, h->rr1, BX, ritz, h->Gtmp, nullptr, m, N));
+      G = h->Gtmp;
+    }
+    RCHFSI_TRY(lambda_table(h, ritz, N, degree, e, c, sigma1, h->lam_table));
+    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RX, 0, el * prec_bytes(pl.store), st));       // R_X <- 0
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, RY, Wcur, m, N));  // R_Y <- (sigma_1/e) G
+    if (need_gs) {
+      RCHFSI_TRY(scale_convert(h, pl.store, 0, 1.0, G, h->Gs, nullptr, m, N));
+      Gst = h->Gs;
+    } else {
+      Gst = G;
+    }
+  } else {
+    // Alg. 2: X_k = X, Y = (sigma_1/e)(D^-1 A (x) X - c X)
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, 1.0, X, RX, Wcur, m, N));
+    const void *W0 = pl.shadow ? Wcur : RX;
+    if (pl.fused) {
+      // first step through the fused kernels: RY <- a T + b X with a = sigma_1/e, b = -a c, c' = 0
+      RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RY, 0, el * prec_bytes(pl.store), st));
+      StepCoef k0{sigma1 / e, -(sigma1 / e) * c, 0.0};
+      RCHFSI_TRY(do_step(h, pl, true, k0, W0, RX, RY, nullptr, nullptr, Wnext, apply_index++));
+    } else {
+      if (pl.tprec == RCHFSI_FP64)
+        RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, (const double *)W0, (double *)h->T, N));
+      else
+        RCHFSI_TRY(op_apply_simt<float>(h, h->A.d, nullptr, (const float *)W0, (float *)h->T, N));
+      if (h->opt.noise_eps > 0)
+        RCHFSI_TRY(add_column_noise(h, pl.tprec, h->T, m, N, h->opt.noise_eps, h->opt.noise_seed, apply_index, h->colnorm));
+      apply_index++;
+      RCHFSI_TRY(chfsi_first(h, pl.store, pl.tprec, pl.operand, sigma1 / e, c, h->T, h->dinv, X, RY, Wnext, m, N));
+    }
+    if (pl.shadow) std::swap(Wcur, Wnext);
+  }
+
+  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step0, st));
+  for (int32_t k = 2; k <= degree; ++k) {
+    const double sigma2 = 1.0 / (gamma - sigma);
+    StepCoef kc{2.0 * sigma2 / e, -2.0 * sigma2 * c / e, -sigma * sigma2};
+    const double *LY = chfsi ? nullptr : h->lam_table + (size_t)(k - 1) * N;
+    const void *W = pl.shadow ? Wcur : RY;
+    RCHFSI_TRY(do_step(h, pl, chfsi, kc, W, RY, RX, chfsi ? nullptr : Gst, LY, Wnext, apply_index++));
+    std::swap(RX, RY);                       // swap(R_X, R_Y)
+    if (pl.shadow) std::swap(Wcur, Wnext);
+    sigma = sigma2;
+  }
+  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step1, st));
+  h->last_steps = degree - 1;
+
+  if (!chfsi)   // Y_p = D^-1 R_Y + X Lambda_Y
+    RCHFSI_TRY(finish_block(h, pl.store, RY, h->dinv, h->lam_table + (size_t)degree * N, X, m, N));
+  else
+    RCHFSI_TRY(finish_block(h, pl.store, RY, nullptr, nullptr, X, m, N));
+  return RCHFSI_OK;
+}
+
+rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host, const double *ritz_host,
+                                 const double *G_host, int32_t degree, double lam_min, double lam_T,
+                                 double lam_max) {
+  if (!h) return RCHFSI_EINVAL;
+  if (!X_host || (method == RCHFSI_METHOD_RCHFSI && !ritz_host)) { h->err = "rchfsi_filter_host: null argument"; return RCHFSI_EINVAL; }
+  const size_t blk = sizeof(double) * (size_t)h->m * h->N;
+  cudaStream_t st = h->stream;
+  if (!h->hX) RCHFSI_TRY(dev_alloc(h, (void **)&h->hX, blk));
+  if (!h->hritz) RCHFSI_TRY(dev_alloc(h, (void **)&h->hritz, sizeof(double) * h->N));
+  if (G_host && !h->hG) RCHFSI_TRY(dev_alloc(h, (void **)&h->hG, blk));
+  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hX, X_host, blk, cudaMemcpyHostToDevice, st));
+  if (ritz_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * h->N, cudaMemcpyHostToDevice, st));
+  if (G_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hG, G_host, blk, cudaMemcpyHostToDevice, st));
+  RCHFSI_TRY(rchfsi_filter(h, method, h->hX, ritz_host ? h->hritz : nullptr, G_host ? h->hG : nullptr, degree,
+                           lam_min, lam_T, lam_max));
+  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(X_host, h->hX, blk, cudaMemcpyDeviceToHost, st));
+  RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
+  return RCHFSI_OK;
+}
+
+rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n_wanted, int32_t degree,
+                           double lam_min, double lam_T, double lam_max, double tol, int32_t max_iter,
+                           double *evals_out, double *resnorm_out, int32_t *iters_out, double *history_out) {
+  if (!h) return RCHFSI_EINVAL;
+  if (!X || !evals_out || !resnorm_out || !iters_out) { h->err = "rchfsi_solve: null argument"; return RCHFSI_EINVAL; }
+  if (n_wanted < 1 || n_wanted > h->N || max_iter < 1 || degree < 1 || !(tol > 0)) { h->err = "rchfsi_solve: bad n_wanted / max_iter / degree / tol"; return RCHFSI_EINVAL; }
+  if (!(lam_min < lam_T) || !(lam_T < lam_max)) { h->err = "rchfsi_solve: need lam_min < lam_T < lam_max"; return RCHFSI_EINVAL; }
+  const int32_t N = h->N;
+  const size_t el = (size_t)h->m * N;
+  cudaStream_t st = h->stream;
+  const bool rch = (method == RCHFSI_METHOD_RCHFSI);
+  if (rch && !h->Gtmp) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gtmp, el * 8));
+  std::vector<double> ritz(N), res(N);
+  // reading S2: one Rayleigh-Ritz on the initial guess gives B-orthonormal X, Lambda and G
+  RCHFSI_TRY(rayleigh_ritz_impl(h, X, h->ritz_dev, rch ? h->Gtmp : nullptr, h->res_dev));
+  rchfsi_status result = RCHFSI_ENOTCONVERGED;
+  int32_t it = 0;
+  for (it = 1; it <= max_iter; ++it) {
+    if (h->opt.adaptive_bounds) {             // reading S7
+      RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz.data(), h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+      RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
+      if (ritz[0] < ritz[N - 1] && ritz[N - 1] < lam_max) { lam_min = ritz[0]; lam_T = ritz[N - 1]; }
+    }
+    RCHFSI_TRY(rchfsi_filter(h, method, X, h->ritz_dev, rch ? h->Gtmp : nullptr, degree, lam_min, lam_T, lam_max));
+    RCHFSI_TRY(rayleigh_ritz_impl(h, X, h->ritz_dev, rch ? h->Gtmp : nullptr, h->res_dev));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(res.data(), h->res_dev, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+    RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
+    double worst = 0.0;
+    for (int j = 0; j < n_wanted; ++j) worst = std::fmax(worst, res[j]);
+    if (history_out) history_out[it - 1] = worst;
+    if (!(worst == worst)) { h->err = "rchfsi_solve: residual is NaN"; result = RCHFSI_EBREAKDOWN; break; }
+    if (worst < tol) { result = RCHFSI_OK; break; }
+  }
+  if (it > max_iter) it = max_iter;
+  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz.data(), h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(res.data(), h->res_dev, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+  RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
+  for (int j = 0; j < N; ++j) { evals_out[j] = ritz[j]; resnorm_out[j] = res[j]; }
+  *iters_out = it;
+  if (result == RCHFSI_ENOTCONVERGED) h->err = "rchfsi_solve: max_iter reached";
+  return result;
+}
+
+}  // extern "C"

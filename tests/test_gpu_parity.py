@@ -1,0 +1,274 @@
+"""GPU parity: the CUDA library (through the C ABI binding) against the FP64 CPU oracle on the
+same seeded inputs.  All-FP64 mode: filtered blocks to <= 1e-10 relative (north_star).  Reduced
+precision modes: converged eigenvalues <= 1e-8 relative and residuals <= 1e-8."""
+import numpy as np
+import pytest
+
+import workloads
+from oracle import chfsi_oracle as orc
+from tests.helpers import oracle_ops, rel_fro, small_dense_generalized
+
+pytestmark = pytest.mark.gpu
+
+TOL_FP64 = 1e-10   # north_star: "relative error <= 1e-10 on filtered blocks in an all-FP64 mode"
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _setup(prob, N, seed, **opts):
+    """Upload the problem, build X (B-orthonormal via the oracle RR), ritz, G on the host."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    A, B, Dinv = oracle_ops(prob)
+    X0 = np.random.default_rng(seed).standard_normal((prob["m"], N))
+    ritz, X, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, X0)
+    G = orc.residual_block(AX, BX, ritz)
+    As, Bs, dinv = P.upload_problem(prob)
+    solver = P.Rchfsi(As, Bs, dinv, block_N=N, **opts)
+    return solver, (A, B, Dinv), X, ritz, G
+
+
+def _bounds(prob, A, B):
+    """Spectral bounds from a library eigensolver on the (small) dense pencil."""
+    import scipy.linalg as sla
+    m = prob["m"]
+    Ad = A.apply(np.eye(m))
+    Bd = B.apply(np.eye(m))
+    ev = sla.eigh(Ad, Bd, eigvals_only=True)
+    dinv = prob.get("dinv")
+    top = ev[-1]
+    if dinv is not None:   # lam_max must also bound lam(D^-1 A) (reading S7)
+        s = np.sqrt(dinv)
+        top = max(top, np.linalg.eigvalsh(s[:, None] * Ad * s[None, :])[-1])
+    return ev, top
+
+
+def _run_filter_parity(prob, N, p, n_inside, method, seed=11):
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    solver, (A, B, Dinv), X, ritz, G = _setup(prob, N, seed)
+    ev, top = _bounds(prob, A, B)
+    lam_min, lam_T, lam_max = ev[0] - 1e-3, ev[n_inside], top * 1.01 + 1e-6
+    if method == "rchfsi":
+        Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, p, lam_min, lam_T, lam_max)
+    else:
+        Yo = orc.filter_chfsi(A.apply, Dinv.apply, X, p, lam_min, lam_T, lam_max)
+    Xd = torch.as_tensor(X).cuda()
+    meth = P.METHOD_RCHFSI if method == "rchfsi" else P.METHOD_CHFSI
+    solver.filter(meth, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, lam_min, lam_T, lam_max)
+    Yg = Xd.cpu().numpy()
+    # column-wise: every column must match, not only the Frobenius norm
+    err = np.linalg.norm(Yg - Yo, axis=0) / np.linalg.norm(Yo, axis=0)
+    assert err.max() <= TOL_FP64, err.max()
+    assert solver.launch_count() > 0
+    if method == "rchfsi":   # G = NULL => the library forms A X - B X Lambda itself
+        Xd2 = torch.as_tensor(X).cuda()
+        solver.filter(meth, Xd2, torch.as_tensor(ritz).cuda(), None, p, lam_min, lam_T, lam_max)
+        # the library's own G differs from the oracle's by rounding of a cancelling difference;
+        # the filter amplifies it by at most C_p'(eps) -- compare loosely
+        assert rel_fro(Xd2.cpu().numpy(), Yo) <= 1e-6
+    solver.close()
+
+
+@pytest.mark.parametrize("method", ["rchfsi", "chfsi"])
+@pytest.mark.parametrize("m,N,p", [(200, 12, 9), (333, 20, 16), (130, 7, 5), (64, 4, 1)])
+def test_dense_generalized_filter_fp64(m, N, p, method):
+    # sizes span several 64-row tiles with ragged tails, N not a multiple of 4, degree 1
+    _run_filter_parity(small_dense_generalized(m, seed=m), N, p, N, method)
+
+
+@pytest.mark.parametrize("method", ["rchfsi", "chfsi"])
+def test_config1_dense_standard_filter_fp64_full_size(method):
+    prob = workloads.config1_dense_standard()
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    N, p = prob["block"], prob["degree"]
+    solver, (A, B, Dinv), X, ritz, G = _setup(prob, N, 5)
+    b = (prob["lam_min"], prob["lam_T"], prob["lam_max"])
+    if method == "rchfsi":
+        Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, p, *b)
+    else:
+        Yo = orc.filter_chfsi(A.apply, Dinv.apply, X, p, *b)
+    Xd = torch.as_tensor(X).cuda()
+    solver.filter(P.METHOD_RCHFSI if method == "rchfsi" else P.METHOD_CHFSI, Xd, torch.as_tensor(ritz).cuda(),
+                  torch.as_tensor(G).cuda(), p, *b)
+    err = np.linalg.norm(Xd.cpu().numpy() - Yo, axis=0) / np.linalg.norm(Yo, axis=0)
+    assert err.max() <= TOL_FP64, err.max()
+    solver.close()
+
+
+@pytest.mark.parametrize("method", ["rchfsi", "chfsi"])
+@pytest.mark.parametrize("n,N,p", [(6, 8, 12), (7, 10, 7), (9, 12, 20)])
+def test_csr_laplacian_filter_fp64(n, N, p, method):
+    prob = workloads.config3_sparse_laplacian(n=n, n_wanted=N - 2, block=N, degree=p, seed=n)
+    _run_filter_parity(prob, N, p, N, method)
+
+
+@pytest.mark.parametrize("method", ["rchfsi", "chfsi"])
+@pytest.mark.parametrize("nc,q,N,p", [(2, 3, 8, 10), (3, 2, 13, 6), (2, 6, 16, 8)])
+def test_fe_generalized_filter_fp64(nc, q, N, p, method):
+    # q=6 is the paper-shaped element (343 nodes per cell); q=2,3 give ragged n_loc = 27, 64
+    prob = workloads.fe_problem(nc, q=q, seed=nc + q)
+    _run_filter_parity(prob, N, p, N, method)
+
+
+def test_rayleigh_ritz_matches_oracle():
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(300, seed=3)
+    N = 24
+    A, B, Dinv = oracle_ops(prob)
+    Y = np.random.default_rng(8).standard_normal((300, N)) * np.logspace(0, 6, N)[None, :]
+    ritz_o, X_o, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, Y)
+    res_o = orc.residual_norms(AX, BX, ritz_o)
+    As, Bs, dinv = P.upload_problem(prob)
+    s = P.Rchfsi(As, Bs, dinv, block_N=N)
+    ritz, X, G, res = s.rayleigh_ritz(torch.as_tensor(Y).cuda())
+    np.testing.assert_allclose(ritz.cpu().numpy(), ritz_o, rtol=1e-11, atol=1e-12)
+    Xg = X.cpu().numpy()
+    # eigenvector signs are free (S12): compare |x_j^T B x_j^oracle| = 1 and B-orthonormality
+    Bd = prob["B"]
+    np.testing.assert_allclose(np.abs(np.sum(Xg * (Bd @ X_o), axis=0)), 1.0, rtol=0, atol=1e-8)
+    np.testing.assert_allclose(Xg.T @ Bd @ Xg, np.eye(N), rtol=0, atol=1e-10)
+    np.testing.assert_allclose(res.cpu().numpy(), res_o, rtol=1e-6, atol=1e-11)
+    Gg = G.cpu().numpy()
+    np.testing.assert_allclose(Gg, prob["A"] @ Xg - (Bd @ Xg) * ritz.cpu().numpy()[None, :], rtol=0, atol=1e-10)
+    # exact operator apply
+    V = torch.as_tensor(Y).cuda()
+    np.testing.assert_allclose(s.apply(0, V).cpu().numpy(), prob["A"] @ Y, rtol=1e-12, atol=1e-6)
+    np.testing.assert_allclose(s.apply(1, V).cpu().numpy(), Bd @ Y, rtol=1e-12, atol=1e-6)
+    s.close()
+
+
+def test_solve_fp64_matches_oracle_solve_iterates_and_eigs():
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.config1_dense_standard(m=400, n_wanted=20, block=24, degree=12, seed=9)
+    A, B, Dinv = oracle_ops(prob)
+    b = (prob["lam_min"], prob["lam_T"], prob["lam_max"])
+    ref = orc.solve(A, B, A, Dinv, prob["X0"], 20, 12, *b, tol=1e-8, max_iter=40)
+    As, Bs, dinv = P.upload_problem(prob)
+    s = P.Rchfsi(As, Bs, dinv, block_N=24)
+    Xd = torch.as_tensor(prob["X0"]).cuda()
+    out = s.solve(P.METHOD_RCHFSI, Xd, 20, 12, *b, tol=1e-8, max_iter=40)
+    assert out["converged"] and out["iters"] == ref["iters"]
+    np.testing.assert_allclose(out["evals"][:20], prob["lam"][:20], rtol=1e-10)
+    np.testing.assert_allclose(out["evals"][:20], ref["evals"][:20], rtol=1e-10)
+    assert out["resnorm"][:20].max() < 1e-8
+    s.close()
+
+
+@pytest.mark.parametrize("apply_prec,store_prec", [("fp32", "fp64"), ("fp32", "fp32"), ("tf32", "fp64"),
+                                                   ("bf16", "fp64"), ("bf16", "fp32")])
+def test_dense_generalized_reduced_precision_solve(apply_prec, store_prec):
+    """Reduced-precision operator apply: converged eigenvalues <= 1e-8 relative to the exact ones,
+    residual <= 1e-8 (north_star); ChFSI with the same inexact apply must not get there."""
+    torch = _torch()
+    import scipy.linalg as sla
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(600, seed=21)
+    N, nw, p = 40, 30, 16
+    ev = sla.eigh(prob["A"], prob["B"], eigvals_only=True)
+    s = np.sqrt(prob["dinv"])
+    top = max(ev[-1], np.linalg.eigvalsh(s[:, None] * prob["A"] * s[None, :])[-1])
+    b = (ev[0] - 1e-2, ev[N], top * 1.02)
+    As, Bs, dinv = P.upload_problem(prob)
+    X0 = np.random.default_rng(1).standard_normal((600, N))
+    sol = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec)
+    out = sol.solve(P.METHOD_RCHFSI, torch.as_tensor(X0).cuda(), nw, p, *b, tol=1e-8, max_iter=60)
+    assert out["converged"], out["history"]
+    np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8)
+    assert out["resnorm"][:nw].max() <= 1e-8
+    sol.close()
+
+
+def test_csr_fp32_fused_solve_matches_oracle_eigs_and_chfsi_stagnates():
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.config3_sparse_laplacian(n=12, n_wanted=24, block=32, degree=20, seed=3)
+    A, B, Dinv = oracle_ops(prob)
+    ev = np.linalg.eigvalsh(A.apply(np.eye(prob["m"])))
+    b = (ev[0] - 1e-2, ev[32], 12.0)
+    As, Bs, dinv = P.upload_problem(prob)
+    X0 = workloads.start_block(prob["m"], 32, prob["x0_seed"])
+    for store in ("fp64", "fp32"):
+        sol = P.Rchfsi(As, Bs, dinv, block_N=32, apply_prec="fp32", store_prec=store)
+        out = sol.solve(P.METHOD_RCHFSI, torch.as_tensor(X0).cuda(), 24, 20, *b, tol=1e-8, max_iter=60)
+        assert out["converged"], (store, out["history"])
+        np.testing.assert_allclose(out["evals"][:24], ev[:24], rtol=1e-8)
+        assert out["resnorm"][:24].max() <= 1e-8
+        sol.close()
+    sol = P.Rchfsi(As, Bs, dinv, block_N=32, apply_prec="fp32", store_prec="fp64")
+    out = sol.solve(P.METHOD_CHFSI, torch.as_tensor(X0).cuda(), 24, 20, *b, tol=1e-8, max_iter=30)
+    assert not out["converged"] and out["history"][-1] > 1e-8    # FP32 ChFSI floors
+    sol.close()
+
+
+def test_csr_fused_step_matches_oracle_within_fp32_error():
+    """One filter in FP32-apply mode is the oracle's filter up to FP32 rounding of the products
+    (Thm 3.4: error proportional to the residual), far below the FP32 error of ChFSI."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.config3_sparse_laplacian(n=10, n_wanted=20, block=24, degree=15, seed=4)
+    solver, (A, B, Dinv), X, ritz, G = _setup(prob, 24, 6, apply_prec="fp32")
+    ev = np.linalg.eigvalsh(A.apply(np.eye(prob["m"])))
+    b = (ev[0] - 1e-2, ev[24], 12.0)
+    Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, 15, *b)
+    Xd = torch.as_tensor(X).cuda()
+    solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), 15, *b)
+    assert rel_fro(Xd.cpu().numpy(), Yo) < 1e-5
+    solver.close()
+
+
+def test_filter_host_entry_point_equals_device_entry_point():
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(150, seed=2)
+    solver, (A, B, Dinv), X, ritz, G = _setup(prob, 8, 3)
+    ev, top = _bounds(prob, A, B)
+    b = (ev[0] - 1e-3, ev[8], top * 1.01)
+    Xd = torch.as_tensor(X).cuda()
+    solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), 7, *b)
+    Xh = X.copy()
+    solver.filter_host(P.METHOD_RCHFSI, Xh, ritz, G, 7, *b)
+    np.testing.assert_array_equal(Xh, Xd.cpu().numpy())
+    solver.close()
+
+
+def test_filter_rejects_bad_arguments_without_touching_X():
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(64, seed=1)
+    solver, _, X, ritz, G = _setup(prob, 4, 3)
+    Xd = torch.as_tensor(X).cuda()
+    rz, Gd = torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda()
+    for args in [(0, 0.0, 1.0, 2.0), (3, 1.0, 1.0, 2.0), (3, 0.0, 2.0, 2.0), (3, 0.0, float("nan"), 2.0)]:
+        with pytest.raises(P.RchfsiError) as ei:
+            solver.filter(P.METHOD_RCHFSI, Xd, rz, Gd, *args)
+        assert ei.value.status == P.EINVAL
+    with pytest.raises(P.RchfsiError):
+        solver.filter(P.METHOD_RCHFSI, Xd, None, Gd, 3, 0.0, 1.0, 2.0)
+    with pytest.raises(P.RchfsiError):
+        solver.filter(7, Xd, rz, Gd, 3, 0.0, 1.0, 2.0)
+    np.testing.assert_array_equal(Xd.cpu().numpy(), X)
+    solver.close()
+
+
+def test_noise_hook_matches_oracle_column_noise():
+    """The library's counter-based generator and column scaling equal workloads.noise +
+    oracle.ColumnNoise, so a noisy FP64 filter is reproduced to rounding."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.config1_dense_standard(m=256, n_wanted=10, block=12, degree=8, seed=3)
+    solver, (A, B, Dinv), X, ritz, G = _setup(prob, 12, 4, noise_eps=1e-4, noise_seed=77)
+    b = (prob["lam_min"], prob["lam_T"], prob["lam_max"])
+    noisy = orc.ColumnNoise(A, 1e-4, lambda k, mm, nn: workloads.counter_gaussian(77, k, mm, nn))
+    Yo = orc.filter_rchfsi(noisy.apply, Dinv.apply, X, ritz, G, 8, *b)
+    Xd = torch.as_tensor(X).cuda()
+    solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), 8, *b)
+    assert rel_fro(Xd.cpu().numpy(), Yo) <= 1e-9
+    solver.close()
