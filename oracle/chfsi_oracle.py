@@ -131,6 +131,25 @@ class ColumnNoise:
         return T + (self.eps * tn / gn)[None, :] * g
 
 
+def operators_from_workload(prob):
+    """(A, B, Dinv) operator objects for a dict made by the `workloads` generators."""
+    kind = prob["kind"]
+    m = prob["m"]
+    if kind == "dense":
+        A = DenseOperator(prob["A"])
+        B = DenseOperator(prob["B"]) if prob.get("B") is not None else ScaledIdentity(m)
+    elif kind == "csr":
+        A = CsrOperator(prob["rowptr"], prob["colind"], prob["vals"], m)
+        B = ScaledIdentity(m)
+    elif kind == "fe":
+        A = FeOperator(prob["A_cells"], prob["conn"], m)
+        B = FeOperator(prob["B_cell"], prob["conn"], m)
+    else:
+        raise ValueError(kind)
+    Dinv = DiagonalInverse(prob["dinv"]) if prob.get("dinv") is not None else ScaledIdentity(m)
+    return A, B, Dinv
+
+
 # --------------------------------------------------------------------------- scalars
 def cheb_scalars(lam_min, lam_T, lam_max):
     """e, c, sigma_1, gamma (first line of Alg. 2 and Alg. 3)."""

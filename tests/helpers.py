@@ -6,21 +6,7 @@ from oracle import chfsi_oracle as orc
 
 def oracle_ops(prob):
     """(A, B, Dinv) oracle operator objects for a workload dict."""
-    kind = prob["kind"]
-    m = prob["m"]
-    if kind == "dense":
-        A = orc.DenseOperator(prob["A"])
-        B = orc.DenseOperator(prob["B"]) if prob.get("B") is not None else orc.ScaledIdentity(m)
-    elif kind == "csr":
-        A = orc.CsrOperator(prob["rowptr"], prob["colind"], prob["vals"], m)
-        B = orc.ScaledIdentity(m)
-    elif kind == "fe":
-        A = orc.FeOperator(prob["A_cells"], prob["conn"], m)
-        B = orc.FeOperator(prob["B_cell"], prob["conn"], m)
-    else:
-        raise ValueError(kind)
-    Dinv = orc.DiagonalInverse(prob["dinv"]) if prob.get("dinv") is not None else orc.ScaledIdentity(m)
-    return A, B, Dinv
+    return orc.operators_from_workload(prob)
 
 
 def rel_fro(a, b):
