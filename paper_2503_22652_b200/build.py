@@ -46,7 +46,7 @@ def build(force=False, verbose=False):
         failed |= p.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    link = [NVCC, "-shared", "-o", LIB] + objs + ["-L/usr/local/cuda/lib64", "-lcublas", "-lcusolver", "-lcuda",
+    link = [NVCC, "-shared", "-o", LIB] + objs + ["-L/usr/local/cuda/lib64", "-lcublas", "-lcusolver",
                                                    "-Xlinker", "-rpath,/usr/local/cuda/lib64"]
     r = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode != 0:

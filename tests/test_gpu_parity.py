@@ -272,3 +272,34 @@ def test_noise_hook_matches_oracle_column_noise():
     solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), 8, *b)
     assert rel_fro(Xd.cpu().numpy(), Yo) <= 1e-9
     solver.close()
+
+
+@pytest.mark.parametrize("apply_prec,tol", [("tf32", 6e-3), ("bf16", 3e-2)])
+@pytest.mark.parametrize("m,N,p", [(600, 40, 3), (1000, 264, 4), (333, 16, 2)])
+def test_dense_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_prec, tol, m, N, p):
+    """tcgen05 path: the residual part D^-1 R_p of the filtered block (Y_p - X Lambda_p) equals the
+    oracle's up to the operand rounding of p-1 <= 3 applies.  Tolerance: per apply the block is
+    truncated to TF32 when it aliases the FP32 R_Y (2^-10) and the operator copy is rounded (2^-11),
+    i.e. <= 1.5e-3 relative; BF16 2^-8 + 2^-9 = 5.9e-3; times 3 applies, rounded up: 6e-3 / 3e-2.
+    Sizes: several 128-column and BN-row tiles, ragged K tail (m not a multiple of 32 / 64)."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(m, seed=m + N)
+    for store in ("fp64", "fp32"):
+        solver, (A, B, Dinv), X, ritz, G = _setup(prob, N, 13, apply_prec=apply_prec, store_prec=store)
+        ev, top = _bounds(prob, A, B)
+        b = (ev[0] - 1e-3, ev[N], top * 1.01)
+        Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, p, *b)
+        XL = X * orc.lambda_recurrence(ritz, p, *b)[p][None, :]
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+        Yg = Xd.cpu().numpy()
+        err = np.linalg.norm((Yg - XL) - (Yo - XL), axis=0) / np.linalg.norm(Yo - XL, axis=0)
+        assert err.max() < tol, (store, err.max())
+        assert err.max() > 1e-9, "suspiciously exact: the reduced-precision path did not run"
+        # CHFSI through the same kernel (dinv applied to the output rows)
+        Yc = orc.filter_chfsi(A.apply, Dinv.apply, X, p, *b)
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_CHFSI, Xd, None, None, p, *b)
+        assert rel_fro(Xd.cpu().numpy(), Yc) < tol
+        solver.close()
