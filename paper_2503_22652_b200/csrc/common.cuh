@@ -1,6 +1,7 @@
 // Internal definitions shared by the translation units of librchfsi.so.
 // Nothing here is visible across the C ABI (include/rchfsi.h).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 #include <cublas_v2.h>
@@ -26,6 +27,15 @@ struct LowpCopy {
   int64_t ld = 0;         // padded K extent (elements)
   int64_t rows_pad = 0;   // padded row extent per matrix
   size_t bytes = 0;
+};
+
+// Cached TMA descriptor (encoding one costs microseconds of host time per step otherwise).
+struct TmapEntry {
+  const void *base;
+  uint64_t rows, cols, pitch;
+  uint32_t box_cols, box_rows;
+  int elem_bytes, bf16, atom32;
+  CUtensorMap map;
 };
 
 struct DeviceOperator {
@@ -65,6 +75,7 @@ struct rchfsi_ctx {
   int32_t lam_table_p = 0;
   double *colnorm = nullptr;              // [2][N]
   std::vector<rchfsi::LowpCopy> lowp;
+  std::vector<rchfsi::TmapEntry> tmaps;
   rchfsi::FeColoring coloring;
 
   // Rayleigh-Ritz workspace

@@ -13,6 +13,7 @@
 //
 // Warp roles (256 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one elected lane),
 // warp 2 = TMEM allocator, warps 4-7 = epilogue (TMEM lane quarter = warp % 4).
+#include <cstdlib>
 #include "common.cuh"
 #include "tc_common.cuh"
 
@@ -42,6 +43,19 @@ bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16,
   return r == CUDA_SUCCESS;
 }
 
+const CUtensorMap *get_tmap_2d(rchfsi_ctx *h, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
+                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32) {
+  for (const TmapEntry &e : h->tmaps)
+    if (e.base == base && e.rows == rows && e.cols == cols && e.pitch == pitch_bytes && e.box_cols == box_cols &&
+        e.box_rows == box_rows && e.elem_bytes == elem_bytes && e.bf16 == (int)bf16 && e.atom32 == (int)atom32)
+      return &e.map;
+  TmapEntry e{base, rows, cols, pitch_bytes, box_cols, box_rows, elem_bytes, (int)bf16, (int)atom32, {}};
+  if (!make_tmap_2d(&e.map, base, elem_bytes, bf16, rows, cols, pitch_bytes, box_cols, box_rows, atom32)) return nullptr;
+  if (h->tmaps.size() > 64) h->tmaps.clear();
+  h->tmaps.push_back(e);
+  return &h->tmaps.back().map;
+}
+
 namespace {
 
 using namespace tc;
@@ -57,16 +71,19 @@ struct DenseTcParams {
   int64_t m;
   int32_t N;
   int32_t num_k_blocks;
+  int32_t debug_mode;   // 0 normal; 1 = no MMA (TMA throughput); 2 = no TMA (MMA throughput): timing probes only
 };
 
 template <int BN>
 struct DenseCfg {
-  static constexpr int W_BYTES = 16384;                 // 128 block columns x 128 B of K per stage
-  static constexpr int A_BYTES = BN * 128;              // BN operator rows x 128 B of K per stage
-  static constexpr int STAGE_BYTES = W_BYTES + A_BYTES;
-  static constexpr int STAGES = (BN >= 256) ? 4 : (BN >= 128 ? 6 : 8);
+  static constexpr int KP = 2;                          // 128-byte K panels per pipeline stage
+  static constexpr int W_BYTES = 16384;                 // 128 block columns x 128 B of K per panel
+  static constexpr int A_BYTES = BN * 128;              // BN operator rows x 128 B of K per panel
+  static constexpr int PANEL_BYTES = W_BYTES + A_BYTES;
+  static constexpr int STAGE_BYTES = KP * PANEL_BYTES;
+  static constexpr int STAGES = (200 * 1024) / STAGE_BYTES < 8 ? (200 * 1024) / STAGE_BYTES : 8;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
-  static constexpr int TMEM_COLS = BN < 32 ? 32 : BN;
+  static constexpr int TMEM_COLS = BN;
 };
 
 template <typename S>
@@ -108,84 +125,123 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == 0) {
-    if (lane == 0) {
-      for (int kb = 0; kb < nkb; ++kb) {
-        const int s = kb % Cfg::STAGES;
-        const uint32_t ph = (kb / Cfg::STAGES) & 1;
-        mbar_wait(empty_bar + s, ph ^ 1);
-        uint8_t *ws = smem + s * Cfg::STAGE_BYTES;
-        uint8_t *as = ws + Cfg::W_BYTES;
-        mbar_expect_tx(full_bar + s, Cfg::STAGE_BYTES);
-        if constexpr (KIND == 0) {
-#pragma unroll
-          for (int a = 0; a < 4; ++a) tma_load_2d(ws + a * 4096, &tmW, full_bar + s, j0 + 32 * a, kb * KR);
+    // ===== TMA producer: the whole warp walks the ring, one elected lane issues =====
+    for (int kb = 0; kb < nkb; ++kb) {
+      const int s = kb % Cfg::STAGES;
+      const uint32_t ph = (kb / Cfg::STAGES) & 1;
+      mbar_wait(empty_bar + s, ph ^ 1);
+      if (elect_one()) {
+        if (p.debug_mode & 2) {
+          mbar_arrive(full_bar + s);
         } else {
+          mbar_expect_tx(full_bar + s, Cfg::STAGE_BYTES);
 #pragma unroll
-          for (int a = 0; a < 2; ++a) tma_load_2d(ws + a * 8192, &tmW, full_bar + s, j0 + 64 * a, kb * KR);
+          for (int pn = 0; pn < Cfg::KP; ++pn) {
+            uint8_t *ws = smem + s * Cfg::STAGE_BYTES + pn * Cfg::PANEL_BYTES;
+            uint8_t *as = ws + Cfg::W_BYTES;
+            const int k0 = (kb * Cfg::KP + pn) * KR;
+            if constexpr (KIND == 0) {
+#pragma unroll
+              for (int a = 0; a < 4; ++a) tma_load_2d(ws + a * 4096, &tmW, full_bar + s, j0 + 32 * a, k0);
+            } else {
+#pragma unroll
+              for (int a = 0; a < 2; ++a) tma_load_2d(ws + a * 8192, &tmW, full_bar + s, j0 + 64 * a, k0);
+            }
+            tma_load_2d(as, &tmA, full_bar + s, k0, (int32_t)i0);
+          }
         }
-        tma_load_2d(as, &tmA, full_bar + s, kb * KR, (int32_t)i0);
       }
+      __syncwarp();
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc(KIND == 0 ? 2 : 1, /*A MN-major*/ 1, /*B K-major*/ 0, 128, BN);
-      for (int kb = 0; kb < nkb; ++kb) {
-        const int s = kb % Cfg::STAGES;
-        const uint32_t ph = (kb / Cfg::STAGES) & 1;
-        mbar_wait(full_bar + s, ph);
-        tc_fence_after();
-        const uint32_t ws = smem_u32(smem + s * Cfg::STAGE_BYTES);
-        const uint32_t as = ws + Cfg::W_BYTES;
+    // ===== MMA issuer =====
+    constexpr uint32_t idesc = make_idesc(KIND == 0 ? 2 : 1, /*A MN-major*/ 1, /*B K-major*/ 0, 128, BN);
+    // W^T tile, MN-major.  TF32: SWIZZLE_128B_BASE32B, 8 k rows per MMA = two 4-row groups (SBO 512 B),
+    // M atoms (32 columns) 4096 B apart.  BF16: SWIZZLE_128B, 16 k rows per MMA = two 8-row groups
+    // (SBO 1024 B), M atoms (64 columns) 8192 B apart.  Operator rows, K-major SWIZZLE_128B: 32 B of K
+    // per MMA inside the 128 B row, 8-row groups 1024 B apart.
+    const uint64_t da0 = (KIND == 0) ? make_smem_desc(smem_u32(smem), 4096, 512, 1) : make_smem_desc(smem_u32(smem), 8192, 1024, 2);
+    const uint64_t db0 = make_smem_desc(smem_u32(smem) + Cfg::W_BYTES, 16, 1024, 2);
+    for (int kb = 0; kb < nkb; ++kb) {
+      const int s = kb % Cfg::STAGES;
+      const uint32_t ph = (kb / Cfg::STAGES) & 1;
+      mbar_wait(full_bar + s, ph);
+      tc_fence_after();
+      if (elect_one()) {
+        if (p.debug_mode & 1) {
+          mbar_arrive(empty_bar + s);
+        } else {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          // W^T tile, MN-major.  TF32: SWIZZLE_128B_BASE32B, 8 k rows per MMA = two 4-row groups
-          // (SBO 512 B), M atoms (32 columns) 4096 B apart.  BF16: SWIZZLE_128B, 16 k rows per MMA =
-          // two 8-row groups (SBO 1024 B), M atoms (64 columns) 8192 B apart.
-          const uint64_t da = (KIND == 0) ? make_smem_desc(ws + q * 1024, 4096, 512, 1)
-                                          : make_smem_desc(ws + q * 2048, 8192, 1024, 2);
-          // operator rows, K-major: 32 B of K per MMA inside the 128 B swizzled row, 8-row groups 1024 B apart
-          const uint64_t db = make_smem_desc(as + q * 32, 16, 1024);
-          umma<KIND>(tmem_base, da, db, idesc, (kb > 0 || q > 0) ? 1u : 0u);
+          for (int pn = 0; pn < Cfg::KP; ++pn) {
+            const uint32_t off = (uint32_t)(s * Cfg::STAGE_BYTES + pn * Cfg::PANEL_BYTES) >> 4;   // 16-byte units
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const uint64_t da = da0 + off + (uint32_t)(q * (KIND == 0 ? 1024 : 2048) >> 4);
+              const uint64_t db = db0 + off + (uint32_t)(q * 32 >> 4);
+              umma<KIND>(tmem_base, da, db, idesc, (kb > 0 || pn > 0 || q > 0) ? 1u : 0u);
+            }
+          }
+          umma_commit(empty_bar + s);
         }
-        umma_commit(empty_bar + s);
       }
-      umma_commit(accum_bar);
+      __syncwarp();
     }
-  } else if (warp >= 4) {
+    if (elect_one()) {
+      if (p.debug_mode & 1) mbar_arrive(accum_bar); else umma_commit(accum_bar);
+    }
+  }
+  __syncwarp();
+  // ---- epilogue: all 8 warps.  Warp w reads TMEM lanes 32 (w % 4) .. +31 (its lane quarter) and the
+  // column half w / 4 of the tile; loads of R_Y, R_X, G for 8 rows are issued before any use.
+  {
     const int q = warp & 3;
+    const int half = warp >> 2;
     const int j = j0 + 32 * q + lane;
     const bool jok = j < p.N;
-    const S *RY = reinterpret_cast<const S *>(p.RY);
-    S *RX = reinterpret_cast<S *>(p.RX);
-    const S *G = reinterpret_cast<const S *>(p.G);
+    const S *__restrict__ RY = reinterpret_cast<const S *>(p.RY);
+    S *__restrict__ RX = reinterpret_cast<S *>(p.RX);
+    const S *__restrict__ G = reinterpret_cast<const S *>(p.G);
     const double ly = (G != nullptr && jok) ? p.LY[j] : 0.0;
     const double ka = p.k.a, kb_ = p.k.b, kc = p.k.cp;
     mbar_wait(accum_bar, 0);
     tc_fence_after();
+    constexpr int HALF_COLS = BN / 2;
 #pragma unroll 1
-    for (int c0 = 0; c0 < BN; c0 += 32) {
+    for (int c0 = half * HALF_COLS; c0 < (half + 1) * HALF_COLS; c0 += 32) {
       uint32_t r[32];
       tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)c0, r);
       tmem_ld_wait();
-      if (!jok) continue;
+      if (!jok || (p.debug_mode & 4)) continue;
 #pragma unroll
-      for (int t = 0; t < 32; ++t) {
-        const int64_t i = i0 + c0 + t;
-        if (i < p.m) {
+      for (int t0 = 0; t0 < 32; t0 += 8) {
+        double ry[8], rx[8], g[8];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          const int64_t i = i0 + c0 + t0 + t;
           const int64_t idx = i * p.N + j;
-          double T = (double)__uint_as_float(r[t]);
-          if (p.dinv_out) T *= p.dinv_out[i];
-          double out = ka * T + kb_ * ld_s(RY + idx) + kc * ld_s(RX + idx);
-          if (G) out += ka * (ld_s(G + idx) * ly);
-          RX[idx] = (S)out;
-          if (p.Wnext) {
-            if constexpr (KIND == 0) {   // round to nearest TF32 here: the MMA itself truncates
-              uint32_t u;
-              asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"((float)out));
-              reinterpret_cast<uint32_t *>(p.Wnext)[idx] = u;
+          const bool ok = i < p.m;
+          ry[t] = ok ? (double)__ldg(RY + idx) : 0.0;
+          rx[t] = ok ? (double)RX[idx] : 0.0;
+          g[t] = (ok && G) ? (double)__ldg(G + idx) : 0.0;
+        }
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          const int64_t i = i0 + c0 + t0 + t;
+          if (i < p.m) {
+            const int64_t idx = i * p.N + j;
+            double T = (double)__uint_as_float(r[t0 + t]);
+            if (p.dinv_out) T *= p.dinv_out[i];
+            const double out = ka * T + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly);
+            RX[idx] = (S)out;
+            if (p.Wnext) {
+              if constexpr (KIND == 0) {   // round to nearest TF32 here: the MMA itself truncates
+                uint32_t u;
+                asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"((float)out));
+                reinterpret_cast<uint32_t *>(p.Wnext)[idx] = u;
+              } else {
+                reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
+              }
             }
-            else
-              reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
           }
         }
       }
@@ -248,7 +304,11 @@ template <int KIND, int BN, typename S>
 rchfsi_status launch_dense(rchfsi_ctx *h, const CUtensorMap &tmW, const CUtensorMap &tmA, const DenseTcParams &p) {
   using Cfg = DenseCfg<BN>;
   auto kern = dense_tc_kernel<KIND, BN, S>;
-  RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+  static bool attr_set = false;
+  if (!attr_set) {
+    RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    attr_set = true;
+  }
   dim3 grid((unsigned)cdiv(p.N, 128), (unsigned)cdiv(p.m, BN));
   kern<<<grid, 256, Cfg::SMEM_BYTES, h->stream>>>(tmW, tmA, p);
   LAUNCH_CHECK(h);
@@ -272,6 +332,10 @@ bool dense_tc_supported(const rchfsi_ctx *h) {
 }
 
 int dense_tc_pick_bn(int64_t m, int32_t N) {
+  if (const char *e = getenv("RCHFSI_DENSE_BN")) {   // tuning knob
+    const int v = atoi(e);
+    if (v == 64 || v == 128 || v == 256) return v;
+  }
   const int64_t tj = cdiv(N, 128);
   if (tj * cdiv(m, 256) >= 120) return 256;
   if (tj * cdiv(m, 128) >= 120) return 128;
@@ -286,15 +350,18 @@ rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
   if (!cp) return st;
   const int eb = bf16 ? 2 : 4;
   const int bn = dense_tc_pick_bn(h->m, h->N);
-  CUtensorMap tmW, tmA;
   // W [m][N]: box = 128 B of block columns x (32 | 64) k rows
-  if (!make_tmap_2d(&tmW, s.W, eb, bf16, (uint64_t)h->m, (uint64_t)h->N, (uint64_t)h->N * eb, bf16 ? 64 : 32, bf16 ? 64 : 32, !bf16) ||
-      !make_tmap_2d(&tmA, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb, bf16 ? 64 : 32, (uint32_t)bn)) {
+  const CUtensorMap *ptW = get_tmap_2d(h, s.W, eb, bf16, (uint64_t)h->m, (uint64_t)h->N, (uint64_t)h->N * eb,
+                                       bf16 ? 64 : 32, bf16 ? 64 : 32, !bf16);
+  const CUtensorMap *ptA = get_tmap_2d(h, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb,
+                                       bf16 ? 64 : 32, (uint32_t)bn);
+  if (!ptW || !ptA) {
     h->err = "cuTensorMapEncodeTiled failed";
     return RCHFSI_ECUDA;
   }
+  const CUtensorMap tmW = *ptW, tmA = *ptA;
   DenseTcParams p{s.k, s.RY, s.RX, s.G, s.LY, s.chfsi ? h->dinv : nullptr, s.Wnext, h->m, h->N,
-                  (int32_t)cdiv(h->m, bf16 ? 64 : 32)};
+                  (int32_t)cdiv(h->m, (bf16 ? 64 : 32) * 2), getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0};
   if (s.store_prec == RCHFSI_FP64)
     return bf16 ? launch_dense_bn<1, double>(h, bn, tmW, tmA, p) : launch_dense_bn<0, double>(h, bn, tmW, tmA, p);
   return bf16 ? launch_dense_bn<1, float>(h, bn, tmW, tmA, p) : launch_dense_bn<0, float>(h, bn, tmW, tmA, p);

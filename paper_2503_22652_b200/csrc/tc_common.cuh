@@ -43,6 +43,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   __trap();
 }
 
+// one lane of a fully converged warp (warp-uniform branch => the compiler sees a single issuer)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred P1;\n\telect.sync _|P1, 0xffffffff;\n\tselp.u32 %0, 1, 0, P1;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
 // ----------------------------------------------------------------------------------- TMA
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap *m) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");
@@ -152,4 +159,11 @@ __host__ __device__ constexpr uint32_t make_idesc(int fmt, int a_mn_major, int b
 bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
                   uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32 = false);
 
+}  // namespace rchfsi
+
+struct rchfsi_ctx;
+namespace rchfsi {
+// cached variant: returns nullptr on failure
+const CUtensorMap *get_tmap_2d(rchfsi_ctx *h, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
+                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32 = false);
 }  // namespace rchfsi
