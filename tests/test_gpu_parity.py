@@ -303,3 +303,33 @@ def test_dense_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_
         solver.filter(P.METHOD_CHFSI, Xd, None, None, p, *b)
         assert rel_fro(Xd.cpu().numpy(), Yc) < tol
         solver.close()
+
+
+@pytest.mark.parametrize("apply_prec,tol", [("tf32", 6e-3), ("bf16", 3e-2)])
+@pytest.mark.parametrize("nc,q,N,p", [(2, 6, 136, 3), (3, 3, 16, 4), (3, 2, 264, 3)])
+def test_fe_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_prec, tol, nc, q, N, p):
+    """FE tcgen05 path (TMA gather4 prologue, coloured atomic-free scatter fused with the update):
+    the residual part of the filtered block equals the oracle's up to operand rounding (tolerances
+    as for the dense kernel).  q=6: 343 nodes per cell, two 176-wide accumulator halves, ragged K
+    tail; q=2,3: single accumulator; N=136/264: a ragged second/third 128-column tile."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.fe_problem(nc, q=q, seed=nc * 10 + q)
+    A, B, Dinv = oracle_ops(prob)
+    lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    for store in ("fp64", "fp32"):
+        solver, _, X, ritz, G = _setup(prob, N, 17, apply_prec=apply_prec, store_prec=store)
+        b = (ritz[0] - 1.0, ritz[-1] + 1.0, lam_max)
+        Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, p, *b)
+        XL = X * orc.lambda_recurrence(ritz, p, *b)[p][None, :]
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+        Yg = Xd.cpu().numpy()
+        err = np.linalg.norm((Yg - XL) - (Yo - XL), axis=0) / np.linalg.norm(Yo - XL, axis=0)
+        assert err.max() < tol, (store, err.max())
+        assert err.max() > 1e-9, "suspiciously exact: the reduced-precision path did not run"
+        Yc = orc.filter_chfsi(A.apply, Dinv.apply, X, p, *b)
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_CHFSI, Xd, None, None, p, *b)
+        assert rel_fro(Xd.cpu().numpy(), Yc) < tol
+        solver.close()
