@@ -37,6 +37,10 @@ WORKLOADS = {
 }
 
 
+FE_CELLS = None
+BLOCK = None
+
+
 def make_problem(wl):
     """Seeded synthetic problem + filter bounds (recipes: DESIGN.md 'Input recipe')."""
     if wl == "c1":
@@ -51,9 +55,17 @@ def make_problem(wl):
         b = (None, None, p["lam_max"])
     elif wl == "c4":
         p = workloads.config4_fe()
+        if FE_CELLS is not None:
+            import workloads.fe as wfe
+            p = wfe.fe_problem(FE_CELLS, 6, 4)
+            p.update(n_wanted=1000, block=1200, degree=40, tol=1e-8, x0_seed=2004)
         b = (None, None, None)
     else:
         raise SystemExit("unknown workload " + wl)
+    if BLOCK is not None:
+        p["block"] = BLOCK
+        p["n_wanted"] = min(p["n_wanted"], BLOCK)
+        p.pop("X0", None)
     return p, b
 
 
@@ -150,7 +162,11 @@ def main():
     ap.add_argument("--store-prec", default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solve", action="store_true")
+    ap.add_argument("--fe-cells", type=int, default=None, help="c4 only: cells per direction (profiling a smaller mesh)")
+    ap.add_argument("--block", type=int, default=None, help="override the block width N (profiling)")
     args = ap.parse_args()
+    global FE_CELLS, BLOCK
+    FE_CELLS, BLOCK = args.fe_cells, args.block
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)

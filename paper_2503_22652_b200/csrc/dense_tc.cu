@@ -201,8 +201,8 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
     const S *__restrict__ RY = reinterpret_cast<const S *>(p.RY);
     S *__restrict__ RX = reinterpret_cast<S *>(p.RX);
     const S *__restrict__ G = reinterpret_cast<const S *>(p.G);
-    const double ly = (G != nullptr && jok) ? p.LY[j] : 0.0;
-    const double ka = p.k.a, kb_ = p.k.b, kc = p.k.cp;
+    const S ly = (S)((G != nullptr && jok) ? p.LY[j] : 0.0);
+    const S ka = (S)p.k.a, kb_ = (S)p.k.b, kc = (S)p.k.cp;
     mbar_wait(accum_bar, 0);
     tc_fence_after();
     constexpr int HALF_COLS = BN / 2;
@@ -214,25 +214,25 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       if (!jok || (p.debug_mode & 4)) continue;
 #pragma unroll
       for (int t0 = 0; t0 < 32; t0 += 8) {
-        double ry[8], rx[8], g[8];
+        S ry[8], rx[8], g[8];
 #pragma unroll
         for (int t = 0; t < 8; ++t) {
           const int64_t i = i0 + c0 + t0 + t;
           const int64_t idx = i * p.N + j;
           const bool ok = i < p.m;
-          ry[t] = ok ? (double)__ldg(RY + idx) : 0.0;
-          rx[t] = ok ? (double)RX[idx] : 0.0;
-          g[t] = (ok && G) ? (double)__ldg(G + idx) : 0.0;
+          ry[t] = ok ? __ldg(RY + idx) : S(0);
+          rx[t] = ok ? RX[idx] : S(0);
+          g[t] = (ok && G) ? __ldg(G + idx) : S(0);
         }
 #pragma unroll
         for (int t = 0; t < 8; ++t) {
           const int64_t i = i0 + c0 + t0 + t;
           if (i < p.m) {
             const int64_t idx = i * p.N + j;
-            double T = (double)__uint_as_float(r[t0 + t]);
-            if (p.dinv_out) T *= p.dinv_out[i];
-            const double out = ka * T + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly);
-            RX[idx] = (S)out;
+            S T = (S)__uint_as_float(r[t0 + t]);
+            if (p.dinv_out) T *= (S)p.dinv_out[i];
+            const S out = ka * T + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly);
+            RX[idx] = out;
             if (p.Wnext) {
               if constexpr (KIND == 0) {   // round to nearest TF32 here: the MMA itself truncates
                 uint32_t u;

@@ -48,10 +48,11 @@ struct FeTcParams {
 };
 
 constexpr int FE_W_BYTES = 16384;
+constexpr int FE_THREADS = 512;   // 16 warps: the epilogue needs memory-level parallelism
 
 // KIND 0: TF32, KIND 1: BF16.  S: storage type of R_X, R_Y, G.
 template <int KIND, typename S>
-__global__ void __launch_bounds__(256, 1) fe_tc_kernel(const __grid_constant__ CUtensorMap tmW,
+__global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_constant__ CUtensorMap tmW,
                                                        const __grid_constant__ CUtensorMap tmA, FeTcParams p) {
   constexpr int KR = KIND == 0 ? 32 : 64;     // k rows per 128-byte panel
   constexpr int KSTEP = KIND == 0 ? 8 : 16;   // k per MMA
@@ -143,8 +144,11 @@ __global__ void __launch_bounds__(256, 1) fe_tc_kernel(const __grid_constant__ C
   }
   __syncwarp();
 
-  // ===== epilogue: all 8 warps; lane quarter = warp % 4, 16-column chunks interleaved over warp / 4 =====
+  // ===== epilogue: all 16 warps; lane quarter = warp % 4, 16-row chunks interleaved over warp / 4.
+  // All loads of a batch (R_X always; R_Y and G on first-touch rows) are issued before any use:
+  // this phase is HBM-bound and lives on bytes in flight.
   {
+    constexpr int BATCH = sizeof(S) == 8 ? 8 : 16;
     const int q4 = warp & 3;
     const int par = warp >> 2;
     const int j = j0 + 32 * q4 + lane;
@@ -152,54 +156,54 @@ __global__ void __launch_bounds__(256, 1) fe_tc_kernel(const __grid_constant__ C
     const S *__restrict__ RY = reinterpret_cast<const S *>(p.RY);
     S *__restrict__ RX = reinterpret_cast<S *>(p.RX);
     const S *__restrict__ G = reinterpret_cast<const S *>(p.G);
-    const double ly = (G != nullptr && jok) ? p.LY[j] : 0.0;
-    const double ka = p.k.a, kb_ = p.k.b, kc = p.k.cp;
+    // the update runs in the storage precision (FP32 storage: FP32 arithmetic)
+    const S ly = (S)((G != nullptr && jok) ? p.LY[j] : 0.0);
+    const S ka = (S)p.k.a, kb_ = (S)p.k.b, kc = (S)p.k.cp;
     mbar_wait(accum_bar, 0);
     tc_fence_after();
     const int nchunks = (p.n_loc + 15) >> 4;
 #pragma unroll 1
-    for (int ch = par; ch < nchunks; ch += 2) {
+    for (int ch = par; ch < nchunks; ch += FE_THREADS / 128) {
       uint32_t r[16];
       tmem_ld_32x16(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(ch * 16), r);
       tmem_ld_wait();
       if (!jok || (p.debug_mode & 4)) continue;
 #pragma unroll
-      for (int t0 = 0; t0 < 16; t0 += 8) {
-        double rx[8], ry[8], g[8];
-        int64_t idx[8];
-        int32_t row[8];
-        uint32_t fl[8];
+      for (int t0 = 0; t0 < 16; t0 += BATCH) {
+        S rx[BATCH], ry[BATCH], g[BATCH];
 #pragma unroll
-        for (int t = 0; t < 8; ++t) {
+        for (int t = 0; t < BATCH; ++t) {
           const int a = ch * 16 + t0 + t;
           const bool ok = a < p.n_loc;
           const int aa = ok ? a : 0;
-          fl[t] = ok ? (uint32_t)flag_s[aa] | 4u : 0u;      // bit2 = valid
-          row[t] = conn_s[aa];
-          idx[t] = (int64_t)row[t] * p.N + j;
-          rx[t] = ok ? (double)RX[idx[t]] : 0.0;
-          const bool first = (fl[t] & 1u) != 0;
-          ry[t] = first ? (double)__ldg(RY + idx[t]) : 0.0;
-          g[t] = (first && G) ? (double)__ldg(G + idx[t]) : 0.0;
+          const bool first = ok && (flag_s[aa] & 1u);
+          const int64_t idx = (int64_t)conn_s[aa] * p.N + j;
+          rx[t] = ok ? RX[idx] : S(0);
+          ry[t] = first ? __ldg(RY + idx) : S(0);
+          g[t] = (first && G) ? __ldg(G + idx) : S(0);
         }
 #pragma unroll
-        for (int t = 0; t < 8; ++t) {
-          if (fl[t] & 4u) {
-            double T = (double)__uint_as_float(r[t0 + t]);
-            if (p.dinv_out) T *= p.dinv_out[row[t]];
-            double out;
-            if (fl[t] & 1u)
+        for (int t = 0; t < BATCH; ++t) {
+          const int a = ch * 16 + t0 + t;
+          if (a < p.n_loc) {
+            const uint32_t flt = flag_s[a];
+            const int32_t rowt = conn_s[a];
+            const int64_t idx = (int64_t)rowt * p.N + j;
+            S T = (S)__uint_as_float(r[t0 + t]);
+            if (p.dinv_out) T *= (S)p.dinv_out[rowt];
+            S out;
+            if (flt & 1u)
               out = ka * T + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly);
             else
               out = rx[t] + ka * T;
-            RX[idx[t]] = (S)out;
-            if (p.Wnext && (fl[t] & 2u)) {
+            RX[idx] = out;
+            if (p.Wnext && (flt & 2u)) {
               if constexpr (KIND == 0) {
                 uint32_t u;
                 asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"((float)out));
-                reinterpret_cast<uint32_t *>(p.Wnext)[idx[t]] = u;
+                reinterpret_cast<uint32_t *>(p.Wnext)[idx] = u;
               } else {
-                reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx[t]] = __float2bfloat16_rn((float)out);
+                reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
               }
             }
           }
