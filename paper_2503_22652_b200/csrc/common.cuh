@@ -157,14 +157,14 @@ rchfsi_status step_elementwise(rchfsi_ctx *h, int store_prec, int t_prec, int sh
                                const StepArgs &a);
 // dst(store) = alpha * src(FP64) (+ shadow), used for R_Y = (sigma_1/e) G and G copies
 rchfsi_status scale_convert(rchfsi_ctx *h, int store_prec, int shadow_prec, double alpha,
-                            const double *src, void *dst, void *shadow, int64_t m, int32_t N);
+                            const double *src, void *dst, void *shadow, int64_t m, int32_t N, int64_t pm = 0);
 // CHFSI first step: Y = alpha * (dinv * T - c X)
 rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_prec, double alpha,
                           double c, const void *T, const double *dinv, const double *X, void *Y,
                           void *shadow, int64_t m, int32_t N);
 // RCHFSI finish: X = dinv * RY + X * LY (PAPER.md:263 last line); CHFSI finish: X = RY
 rchfsi_status finish_block(rchfsi_ctx *h, int store_prec, const void *RY, const double *dinv,
-                           const double *LY, double *X, int64_t m, int32_t N);
+                           const double *LY, double *X, int64_t m, int32_t N, int64_t pm = 0);
 // FP64 -> operand precision shadow of X (CHFSI start)
 rchfsi_status convert_block(rchfsi_ctx *h, int dst_prec, const double *src, void *dst, int64_t m,
                             int32_t N);

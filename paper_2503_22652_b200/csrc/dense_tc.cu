@@ -20,7 +20,7 @@
 namespace rchfsi {
 
 bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
-                  uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32) {
+                  uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32) {
   typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -36,15 +36,17 @@ bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16,
   cuuint32_t box[2] = {box_cols, box_rows};
   cuuint32_t estr[2] = {1, 1};
   CUtensorMapDataType dt = bf16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
-                                : (elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT8);
+                                : (elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                                                   : (elem_bytes == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_UINT8));
   CUresult r = encode(out, dt, 2, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                      atom32 ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : CU_TENSOR_MAP_SWIZZLE_128B,
+                      atom32 == 2 ? CU_TENSOR_MAP_SWIZZLE_NONE
+                                  : (atom32 == 1 ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : CU_TENSOR_MAP_SWIZZLE_128B),
                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS;
 }
 
 const CUtensorMap *get_tmap_2d(rchfsi_ctx *h, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
-                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32) {
+                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32) {
   for (const TmapEntry &e : h->tmaps)
     if (e.base == base && e.rows == rows && e.cols == cols && e.pitch == pitch_bytes && e.box_cols == box_cols &&
         e.box_rows == box_rows && e.elem_bytes == elem_bytes && e.bf16 == (int)bf16 && e.atom32 == (int)atom32)

@@ -128,7 +128,9 @@ template <int VEC>
 __global__ void __launch_bounds__(256) misc_kernel(int mode, double alpha, double c, const void *T, int t_prec,
                                                    const double *dinv, const double *LY, const double *src,
                                                    void *dst, int dst_prec, void *shadow, int shadow_prec,
-                                                   int64_t m, int32_t N) {
+                                                   int64_t m, int32_t N, int64_t pm) {
+  // pm != 0: the library-owned blocks (R_X / R_Y / G copy / shadows) are stored in PANEL layout
+  // [ceil(N/128)][m][128] (see fe_tc.cu); user blocks (X, G) are always row-major [m][N].
   const int nv = N / VEC;
   const int64_t total = m * nv;
   for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total;
@@ -136,6 +138,7 @@ __global__ void __launch_bounds__(256) misc_kernel(int mode, double alpha, doubl
     const int64_t row = t / nv;
     const int j = (int)(t - row * nv) * VEC;
     const int64_t idx = row * N + j;
+    const int64_t lidx = pm ? (((int64_t)(j >> 7) * pm + row) << 7) + (j & 127) : idx;
     Vals<VEC> out;
     if (mode == 0) {
       Vals<VEC> s = ld_vec<VEC>(src, idx, RCHFSI_FP64);
@@ -149,35 +152,35 @@ __global__ void __launch_bounds__(256) misc_kernel(int mode, double alpha, doubl
       for (int q = 0; q < VEC; ++q) out.v[q] = alpha * (ds * tt.v[q] - c * s.v[q]);
     } else if (mode == 2) {
       Vals<VEC> x = ld_vec<VEC>(dst, idx, RCHFSI_FP64);
-      Vals<VEC> ry = ld_vec<VEC>(T, idx, t_prec);
+      Vals<VEC> ry = ld_vec<VEC>(T, lidx, t_prec);
       const double ds = dinv ? dinv[row] : 1.0;
 #pragma unroll
       for (int q = 0; q < VEC; ++q) out.v[q] = ds * ry.v[q] + x.v[q] * LY[j + q];
     } else {
-      out = ld_vec<VEC>(T, idx, t_prec);
+      out = ld_vec<VEC>(T, lidx, t_prec);
     }
-    st_vec<VEC>(dst, idx, dst_prec, out);
-    if (shadow) st_vec<VEC>(shadow, idx, shadow_prec, out);
+    st_vec<VEC>(dst, mode == 0 ? lidx : idx, dst_prec, out);
+    if (shadow) st_vec<VEC>(shadow, lidx, shadow_prec, out);
   }
 }
 
 static rchfsi_status launch_misc(rchfsi_ctx *h, int mode, double alpha, double c, const void *T, int t_prec,
                                  const double *dinv, const double *LY, const double *src, void *dst,
-                                 int dst_prec, void *shadow, int shadow_prec, int64_t m, int32_t N) {
+                                 int dst_prec, void *shadow, int shadow_prec, int64_t m, int32_t N, int64_t pm = 0) {
   if (N % 4 == 0)
     misc_kernel<4><<<ew_grid(m * (N / 4)), 256, 0, h->stream>>>(mode, alpha, c, T, t_prec, dinv, LY, src, dst,
-                                                                 dst_prec, shadow, shadow_prec, m, N);
+                                                                 dst_prec, shadow, shadow_prec, m, N, pm);
   else
     misc_kernel<1><<<ew_grid(m * N), 256, 0, h->stream>>>(mode, alpha, c, T, t_prec, dinv, LY, src, dst,
-                                                           dst_prec, shadow, shadow_prec, m, N);
+                                                           dst_prec, shadow, shadow_prec, m, N, pm);
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }
 
 rchfsi_status scale_convert(rchfsi_ctx *h, int store_prec, int shadow_prec, double alpha,
-                            const double *src, void *dst, void *shadow, int64_t m, int32_t N) {
+                            const double *src, void *dst, void *shadow, int64_t m, int32_t N, int64_t pm) {
   return launch_misc(h, 0, alpha, 0.0, nullptr, 0, nullptr, nullptr, src, dst, store_prec, shadow,
-                     shadow_prec, m, N);
+                     shadow_prec, m, N, pm);
 }
 rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_prec, double alpha,
                           double c, const void *T, const double *dinv, const double *X, void *Y,
@@ -185,8 +188,8 @@ rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_
   return launch_misc(h, 1, alpha, c, T, t_prec, dinv, nullptr, X, Y, store_prec, shadow, shadow_prec, m, N);
 }
 rchfsi_status finish_block(rchfsi_ctx *h, int store_prec, const void *RY, const double *dinv,
-                           const double *LY, double *X, int64_t m, int32_t N) {
-  return launch_misc(h, LY ? 2 : 3, 0.0, 0.0, RY, store_prec, dinv, LY, nullptr, X, RCHFSI_FP64, nullptr, 0, m, N);
+                           const double *LY, double *X, int64_t m, int32_t N, int64_t pm) {
+  return launch_misc(h, LY ? 2 : 3, 0.0, 0.0, RY, store_prec, dinv, LY, nullptr, X, RCHFSI_FP64, nullptr, 0, m, N, pm);
 }
 rchfsi_status convert_block(rchfsi_ctx *h, int dst_prec, const double *src, void *dst, int64_t m,
                             int32_t N) {

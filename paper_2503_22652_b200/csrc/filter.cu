@@ -13,6 +13,7 @@ struct Plan {
   int tprec;     // precision of the unfused operator output T
   bool shadow;   // operand block is a separate buffer
   int fused;     // 0 unfused SIMT, 1 CSR fused, 2 dense tensor-core, 3 FE tensor-core
+  bool panel;    // library-owned blocks in panel layout [ceil(N/128)][m][128] (FE tensor-core path)
 };
 
 Plan make_plan(const rchfsi_ctx *h) {
@@ -34,11 +35,12 @@ Plan make_plan(const rchfsi_ctx *h) {
   }
   p.tprec = (ap == RCHFSI_FP64) ? RCHFSI_FP64 : RCHFSI_FP32;
   p.shadow = (p.operand != p.store);
+  p.panel = (p.fused == 3);
   return p;
 }
 
 rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t degree, bool need_gs) {
-  const size_t el = (size_t)h->m * h->N;
+  const size_t el = (size_t)h->m * (pl.panel ? (size_t)cdiv(h->N, 128) * 128 : (size_t)h->N);
   if (!h->RX) RCHFSI_TRY(dev_alloc(h, &h->RX, el * prec_bytes(pl.store)));
   if (!h->RY) RCHFSI_TRY(dev_alloc(h, &h->RY, el * prec_bytes(pl.store)));
   if (pl.shadow) {
@@ -99,7 +101,9 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   const int32_t N = h->N;
   const size_t el = (size_t)m * N;
   cudaStream_t st = h->stream;
-  const bool need_gs = !chfsi && pl.store != RCHFSI_FP64;
+  const bool need_gs = !chfsi && (pl.store != RCHFSI_FP64 || pl.panel);
+  const int64_t pm = pl.panel ? m : 0;
+  const size_t el_lib = pl.panel ? (size_t)m * (size_t)cdiv(N, 128) * 128 : el;
   RCHFSI_TRY(ensure_filter_workspace(h, pl, degree, need_gs));
 
   // first line of Alg. 2 / Alg. 3
@@ -129,21 +133,21 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
       G = h->Gtmp;
     }
     RCHFSI_TRY(lambda_table(h, ritz, N, degree, e, c, sigma1, h->lam_table));
-    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RX, 0, el * prec_bytes(pl.store), st));       // R_X <- 0
-    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, RY, Wcur, m, N));  // R_Y <- (sigma_1/e) G
+    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RX, 0, el_lib * prec_bytes(pl.store), st));       // R_X <- 0
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, RY, Wcur, m, N, pm));  // R_Y <- (sigma_1/e) G
     if (need_gs) {
-      RCHFSI_TRY(scale_convert(h, pl.store, 0, 1.0, G, h->Gs, nullptr, m, N));
+      RCHFSI_TRY(scale_convert(h, pl.store, 0, 1.0, G, h->Gs, nullptr, m, N, pm));
       Gst = h->Gs;
     } else {
       Gst = G;
     }
   } else {
     // Alg. 2: X_k = X, Y = (sigma_1/e)(D^-1 A (x) X - c X)
-    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, 1.0, X, RX, Wcur, m, N));
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, 1.0, X, RX, Wcur, m, N, pm));
     const void *W0 = pl.shadow ? Wcur : RX;
     if (pl.fused) {
       // first step through the fused kernels: RY <- a T + b X with a = sigma_1/e, b = -a c, c' = 0
-      RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RY, 0, el * prec_bytes(pl.store), st));
+      RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RY, 0, el_lib * prec_bytes(pl.store), st));
       StepCoef k0{sigma1 / e, -(sigma1 / e) * c, 0.0};
       RCHFSI_TRY(do_step(h, pl, true, k0, W0, RX, RY, nullptr, nullptr, Wnext, apply_index++));
     } else {
@@ -174,9 +178,9 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   h->last_steps = degree - 1;
 
   if (!chfsi)   // Y_p = D^-1 R_Y + X Lambda_Y
-    RCHFSI_TRY(finish_block(h, pl.store, RY, h->dinv, h->lam_table + (size_t)degree * N, X, m, N));
+    RCHFSI_TRY(finish_block(h, pl.store, RY, h->dinv, h->lam_table + (size_t)degree * N, X, m, N, pm));
   else
-    RCHFSI_TRY(finish_block(h, pl.store, RY, nullptr, nullptr, X, m, N));
+    RCHFSI_TRY(finish_block(h, pl.store, RY, nullptr, nullptr, X, m, N, pm));
   return RCHFSI_OK;
 }
 

@@ -71,6 +71,17 @@ __device__ __forceinline__ void tma_gather4(void *smem_dst, const CUtensorMap *m
       : "memory");
 }
 
+// ------------------------------------------------------------------- cp.async (LDGSTS)
+// 16-byte global -> shared copy; src_bytes = 0 zero-fills the destination without reading
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
 // ------------------------------------------------------------------------------- tcgen05
 __device__ __forceinline__ void tmem_alloc(uint32_t *smem_result, uint32_t ncols) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_result)), "r"(ncols)
@@ -126,6 +137,18 @@ __device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t (&r)[16])
       : "r"(taddr)
       : "memory");
 }
+__device__ __forceinline__ void tmem_ld_32x8(uint32_t taddr, uint32_t (&r)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr)
+               : "memory");
+}
+__device__ __forceinline__ void tmem_ld_32x4(uint32_t taddr, uint32_t (&r)[4]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(taddr)
+               : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // --------------------------------------------------------------------------- descriptors
@@ -154,10 +177,10 @@ __host__ __device__ constexpr uint32_t make_idesc(int fmt, int a_mn_major, int b
 
 // ---- host side: tensor maps (driver API through the runtime's entry-point lookup) ----------
 // 2D row-major tensor [rows][cols] of elem_bytes elements, row pitch in bytes, box {box_cols, box_rows},
-// SWIZZLE_128B (or, atom32 = true, SWIZZLE_128B_ATOM_32B); box_cols * elem_bytes must be 128;
-// OOB reads return zero.
+// SWIZZLE_128B (or, atom32 = 1, SWIZZLE_128B_ATOM_32B; atom32 = 2: no swizzle, any box width); with a
+// swizzle box_cols * elem_bytes must be 128; OOB reads return zero.  elem_bytes 8 = FP64.
 bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
-                  uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32 = false);
+                  uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32 = 0);
 
 }  // namespace rchfsi
 
@@ -165,5 +188,5 @@ struct rchfsi_ctx;
 namespace rchfsi {
 // cached variant: returns nullptr on failure
 const CUtensorMap *get_tmap_2d(rchfsi_ctx *h, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
-                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, bool atom32 = false);
+                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32 = 0);
 }  // namespace rchfsi
