@@ -110,10 +110,13 @@ def oracle_filter_time(prob, X, ritz, G, p, bounds, max_cols):
     from oracle import chfsi_oracle as orc
     A, B, Dinv = orc.operators_from_workload(prob)
     nc = min(max_cols, X.shape[1])
-    t0 = time.perf_counter()
-    orc.filter_rchfsi(A.apply, Dinv.apply, X[:, :nc].copy(), ritz[:nc], G[:, :nc].copy(), p, *bounds)
-    dt = time.perf_counter() - t0
-    return prob["m"] * nc * p / dt, nc, dt
+    reps, dt = 0, 0.0
+    while reps < 1 or (dt < 5.0 and reps < 20):     # a bounded sample: at least one filter, ~5-30 s of CPU work
+        t0 = time.perf_counter()
+        orc.filter_rchfsi(A.apply, Dinv.apply, X[:, :nc].copy(), ritz[:nc], G[:, :nc].copy(), p, *bounds)
+        dt += time.perf_counter() - t0
+        reps += 1
+    return prob["m"] * nc * p * reps / dt, nc, dt
 
 
 def run_reference(args):
@@ -239,14 +242,13 @@ def main():
     launches = solver.launch_count() - l0
     sampler.stop_flag = True
     sampler.join(timeout=2)
+    from paper_2503_22652_b200.sharding import reduce_job
     total_ms = sum(a.elapsed_time(bb) for a, bb in ev)
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.barrier()
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    # max over ranks of the device time, sum over ranks of the units (column shards, no data-path collective)
+    total_ms, updates = reduce_job(total_ms, float(m) * N * p)
     ms_per_step = total_ms / args.steps
-    updates = float(m) * N * p * world
     value = updates / (ms_per_step * 1e-3)
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
@@ -308,6 +310,12 @@ def main():
         roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                 "traffic": None, "kernel": "fused operator + recurrence step", "peak_source": peak_src}
     roof["step_launch_ms"] = step_ms
+    try:   # DRAM bytes per step from the committed ncu --set full capture of this configuration, else null
+        tr = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))
+        if FE_CELLS is None and BLOCK is None:
+            roof["traffic"] = tr.get("%s:%s:%s" % (args.workload, apply_prec, store_prec))
+    except Exception:
+        pass
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
