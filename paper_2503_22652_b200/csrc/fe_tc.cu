@@ -3,7 +3,8 @@
 //   T_c[a][j] = sum_b A_c[a][b] W[conn_c[b]][j]
 // on tcgen05 (kind::tf32 / kind::f16 BF16, FP32 accumulate in TMEM) with
 //   * the GATHER fused into the prologue: the rows conn_c[b] of the operand block W are fetched by
-//     TMA tile::gather4 straight into the swizzled MN-major operand layout (no gathered copy);
+//     16-byte cp.async straight into the swizzled MN-major operand layout (no gathered copy; TMA
+//     tile::gather4 does the same but retires only ~1 op per 100 cycles per SM, see below);
 //   * an ATOMIC-FREE scatter-add fused with the Alg. 3 update: the cells are
 //     coloured so that cells of one colour share no node; colours run as stream-ordered launches.
 //     The update is linear in T, so the first cell touching a node writes
@@ -162,6 +163,12 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
       };
       for (int pn = 0; pn < npanels; ++pn) {
         const int s = pn % FE_STAGES;
+        // publish panel pn-2 BEFORE blocking on the slot of panel pn: otherwise the full barrier of
+        // pn-2 would wait for the MMAs of pn-3 to COMPLETE and every panel would pay a barrier round trip
+        if (pn >= FE_STAGES - 1) {
+          cp_async_wait<FE_STAGES - 2>();
+          arrive_panel(pn - (FE_STAGES - 1));
+        }
         mbar_wait(empty_bar + s, ((pn / FE_STAGES) & 1) ^ 1);
         uint8_t *ws = smem + s * stage_bytes;
 #pragma unroll
@@ -190,10 +197,6 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
           cp_async16(ws + dst_off, Wb + ((uint64_t)rowp * 128 + (ok ? cl : 0)) * EB, ok ? 16u : 0u);
         }
         cp_async_commit();
-        if (pn >= FE_STAGES - 1) {
-          cp_async_wait<FE_STAGES - 1>();
-          arrive_panel(pn - (FE_STAGES - 1));
-        }
       }
       cp_async_wait<0>();
       for (int pn = max(0, npanels - (FE_STAGES - 1)); pn < npanels; ++pn) arrive_panel(pn);
