@@ -56,7 +56,7 @@ typedef enum { RCHFSI_OP_DENSE = 0, RCHFSI_OP_CSR = 1, RCHFSI_OP_FE = 2 } rchfsi
  * computation of A D^-1 R_Y is done using FP32 arithmetic", TF32 compute mode, BF16).
  * FP64: exact products (parity mode).  FP32: FP32 operands, FP32 FMA on the ALUs.
  * TF32 / BF16: tensor-core operands, FP32 accumulate (dense and FE operators; a CSR
- * operator treats TF32 as FP32 and BF16 as BF16-stored block with FP32 FMA). */
+ * operator runs TF32 and BF16 requests as FP32: the sparse product is on the ALUs). */
 typedef enum { RCHFSI_FP64 = 0, RCHFSI_FP32 = 1, RCHFSI_TF32 = 2, RCHFSI_BF16 = 3 } rchfsi_prec;
 
 /* RCHFSI_METHOD_CHFSI: Algorithm 2 with H = D^-1 (A (x) .)  (eq. (7) at 170).
@@ -104,7 +104,8 @@ typedef struct {
                                  T_j += eps ||T_j|| g_j/||g_j|| inside the filter only
                                  (BASELINE.json configs[0]; reading S11) */
   uint64_t noise_seed;
-  int32_t use_cuda_graph;     /* capture the p-1 recurrence steps in a CUDA graph */
+  int32_t use_cuda_graph;     /* reserved (ignored): the step coefficients are kernel arguments, so a graph
+                                 would have to be re-captured per call; measured launch gaps are < 2 us */
   int32_t reserved;
 } rchfsi_options;
 

@@ -5,6 +5,8 @@
 // are read once, R_X is written once.  The operand W is R_Y itself (converted to FP32 on the
 // fly when the recurrence is stored in FP64); D^-1 is folded into the FP32 copy of the values
 // (a_it * dinv[col_t]), which is exact algebra for A D^-1 ("A D^-1 R_Y").
+#include <cstdlib>
+#include <type_traits>
 #include "common.cuh"
 
 namespace rchfsi {
@@ -123,17 +125,26 @@ rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s) {
     h->lowp.push_back(c);
     cp = &h->lowp.back();
   }
-  constexpr int ROWS = 32;
-  const unsigned grid = (unsigned)cdiv(h->m, ROWS);
   const double *dinv_out = s.chfsi ? h->dinv : nullptr;
-  if (s.store_prec == RCHFSI_FP64)
-    csr_fused_kernel<double, ROWS><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
-                                                                 (const double *)s.RY, (double *)s.RX,
-                                                                 (const double *)s.G, s.LY, s.k, h->m, h->N);
-  else
-    csr_fused_kernel<float, ROWS><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
-                                                                (const float *)s.RY, (float *)s.RX,
-                                                                (const float *)s.G, s.LY, s.k, h->m, h->N);
+  int rows = 32;
+  if (const char *e = getenv("RCHFSI_CSR_ROWS")) rows = atoi(e);   // tuning knob
+  auto launch = [&](auto rows_tag) {
+    constexpr int ROWS = decltype(rows_tag)::value;
+    const unsigned grid = (unsigned)cdiv(h->m, ROWS);
+    if (s.store_prec == RCHFSI_FP64)
+      csr_fused_kernel<double, ROWS><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
+                                                                   (const double *)s.RY, (double *)s.RX,
+                                                                   (const double *)s.G, s.LY, s.k, h->m, h->N);
+    else
+      csr_fused_kernel<float, ROWS><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
+                                                                  (const float *)s.RY, (float *)s.RX,
+                                                                  (const float *)s.G, s.LY, s.k, h->m, h->N);
+  };
+  if (rows == 8) launch(std::integral_constant<int, 8>{});
+  else if (rows == 16) launch(std::integral_constant<int, 16>{});
+  else if (rows == 64) launch(std::integral_constant<int, 64>{});
+  else if (rows == 128) launch(std::integral_constant<int, 128>{});
+  else launch(std::integral_constant<int, 32>{});
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }

@@ -333,3 +333,57 @@ def test_fe_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_pre
         solver.filter(P.METHOD_CHFSI, Xd, None, None, p, *b)
         assert rel_fro(Xd.cpu().numpy(), Yc) < tol
         solver.close()
+
+
+@pytest.mark.parametrize("kind", ["dense", "fe"])
+@pytest.mark.parametrize("apply_prec", ["tf32", "bf16"])
+def test_tensor_core_paths_edge_shapes(kind, apply_prec):
+    """Degenerate shapes through the tcgen05 kernels: a problem smaller than one tile (m < 64 rows,
+    N = 8 columns < 128), degree 1 (no step launch at all) and degree 2 (a single step)."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    if kind == "dense":
+        prob = small_dense_generalized(40, seed=5)
+        lam_max_extra = None
+    else:
+        prob = workloads.fe_problem(1, q=2, seed=3)      # one cell, 27 nodes
+        lam_max_extra = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    A, B, Dinv = oracle_ops(prob)
+    N = 8
+    tol = 6e-3 if apply_prec == "tf32" else 3e-2
+    for p in (1, 2):
+        solver, _, X, ritz, G = _setup(prob, N, 23, apply_prec=apply_prec)
+        if lam_max_extra is None:
+            ev, top = _bounds(prob, A, B)
+            b = (ev[0] - 1e-3, ev[N], top * 1.01)
+        else:
+            b = (ritz[0] - 1.0, ritz[-1] + 1.0, lam_max_extra)
+        Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, p, *b)
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+        err = rel_fro(Xd.cpu().numpy(), Yo)
+        assert err < (1e-12 if p == 1 else tol), (p, err)      # degree 1 has no operator apply: exact
+        solver.close()
+
+
+def test_fe_tensor_core_solve_converges_to_exact_eigenvalues():
+    """Whole R-ChFSI solve through the fused FE tcgen05 step (TF32 and BF16 operands, FP32 storage = the
+    paper's scheme): eigenvalues <= 1e-8 relative, residual <= 1e-8 (north_star)."""
+    torch = _torch()
+    import scipy.linalg as sla
+    import paper_2503_22652_b200 as P
+    prob = workloads.fe_problem(2, q=4, seed=11)           # 8 cells, 125 nodes per cell, 729 nodes
+    A, B, Dinv = oracle_ops(prob)
+    m = prob["m"]
+    ev = sla.eigh(A.apply(np.eye(m)), B.apply(np.eye(m)), eigvals_only=True)
+    lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    N, nw, p = 16, 8, 30
+    X0 = np.random.default_rng(2).standard_normal((m, N))
+    As, Bs, dinv = P.upload_problem(prob)
+    for apply_prec in ("tf32", "bf16"):
+        sol = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec="fp32", adaptive_bounds=True)
+        out = sol.solve(P.METHOD_RCHFSI, torch.as_tensor(X0).cuda(), nw, p, ev[0] - 1.0, ev[N] , lam_max, tol=1e-8, max_iter=80)
+        assert out["converged"], (apply_prec, out["history"][-5:])
+        np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8, atol=1e-9)
+        assert out["resnorm"][:nw].max() <= 1e-8
+        sol.close()
