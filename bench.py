@@ -186,6 +186,7 @@ def main():
     ap.add_argument("--store-prec", default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solve", action="store_true")
+    ap.add_argument("--solve", action="store_true", help="also run rchfsi_solve on c4 (about a minute)")
     ap.add_argument("--fe-cells", type=int, default=None, help="c4 only: cells per direction (profiling a smaller mesh)")
     ap.add_argument("--block", type=int, default=None, help="override the block width N (profiling)")
     args = ap.parse_args()
@@ -350,7 +351,7 @@ def main():
                    "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},
            "roofline": roof, "wall_s_timed_region": t_wall}
 
-    if not args.no_solve and args.workload in ("c1", "c2", "c3"):
+    if not args.no_solve and (args.workload in ("c1", "c2", "c3") or args.solve):
         Xs = torch.as_tensor(X0, dtype=torch.float64).to(dev)
         so = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec,
                       adaptive_bounds=(args.workload != "c1"), **noise)

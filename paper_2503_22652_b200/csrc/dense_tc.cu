@@ -73,6 +73,7 @@ struct DenseTcParams {
   int64_t m;
   int32_t N;
   int32_t num_k_blocks;
+  int32_t ksplit;       // K splits = cluster size along z (1, 2, 4 or 8)
   int32_t debug_mode;   // 0 normal; 1 = no MMA (TMA throughput); 2 = no TMA (MMA throughput): timing probes only
 };
 
@@ -108,7 +109,10 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
   const int lane = threadIdx.x & 31;
   const int j0 = blockIdx.x * 128;
   const int64_t i0 = (int64_t)blockIdx.y * BN;
-  const int nkb = p.num_k_blocks;
+  // split-K: the gridDim.z CTAs of a cluster share one output tile; CTA z accumulates its K slice
+  const int ks = gridDim.z;
+  const int kb_begin = (int)((int64_t)p.num_k_blocks * blockIdx.z / ks);
+  const int nkb = (int)((int64_t)p.num_k_blocks * (blockIdx.z + 1) / ks) - kb_begin;
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmW);
@@ -141,7 +145,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
           for (int pn = 0; pn < Cfg::KP; ++pn) {
             uint8_t *ws = smem + s * Cfg::STAGE_BYTES + pn * Cfg::PANEL_BYTES;
             uint8_t *as = ws + Cfg::W_BYTES;
-            const int k0 = (kb * Cfg::KP + pn) * KR;
+            const int k0 = ((kb_begin + kb) * Cfg::KP + pn) * KR;
             if constexpr (KIND == 0) {
 #pragma unroll
               for (int a = 0; a < 4; ++a) tma_load_2d(ws + a * 4096, &tmW, full_bar + s, j0 + 32 * a, k0);
@@ -208,6 +212,72 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
     mbar_wait(accum_bar, 0);
     tc_fence_after();
     constexpr int HALF_COLS = BN / 2;
+    if (ks > 1) {
+      // ---- split-K fix-up over distributed shared memory: every CTA of the cluster parks its partial
+      // tile in its own shared memory ([matrix row][128 columns] FP32, over the dead operand stages),
+      // then CTA z sums the BN / ks matrix rows it owns over the ranks in fixed order (deterministic)
+      // and applies the update to them.
+      float *part = reinterpret_cast<float *>(smem);
+#pragma unroll 1
+      for (int c0 = half * HALF_COLS; c0 < (half + 1) * HALF_COLS; c0 += 32) {
+        uint32_t r[32];
+        tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)c0, r);
+        tmem_ld_wait();
+#pragma unroll
+        for (int t = 0; t < 32; ++t) part[(c0 + t) * 128 + 32 * q + lane] = __uint_as_float(r[t]);
+      }
+      cluster_sync_all();
+      const int jl = threadIdx.x & 127;
+      const int jj = j0 + jl;
+      const bool jjok = jj < p.N;
+      const S ly2 = (S)((G != nullptr && jjok) ? p.LY[jj] : 0.0);
+      const int cpr = BN / ks;                                  // matrix rows owned by this CTA
+      const int cbase = blockIdx.z * cpr + (threadIdx.x >> 7);  // this thread: every second owned row
+      const uint32_t part_s = smem_u32(part);
+      if (jjok && !(p.debug_mode & 4)) {
+#pragma unroll 1
+        for (int u0 = 0; u0 < cpr / 2; u0 += 8) {
+          S ry[8], rx[8], g[8];
+          float T[8];
+#pragma unroll
+          for (int t = 0; t < 8; ++t) {
+            const int c = cbase + 2 * (u0 + t);
+            const int64_t i = i0 + c;
+            const int64_t idx = i * p.N + jj;
+            const bool ok = (u0 + t) < cpr / 2 && i < p.m;
+            ry[t] = ok ? __ldg(RY + idx) : S(0);
+            rx[t] = ok ? RX[idx] : S(0);
+            g[t] = (ok && G) ? __ldg(G + idx) : S(0);
+            float acc = 0.f;
+            if (ok)
+              for (int rr = 0; rr < ks; ++rr) acc += dsmem_ld_f32(dsmem_map(part_s, rr) + (uint32_t)(c * 128 + jl) * 4u);
+            T[t] = acc;
+          }
+#pragma unroll
+          for (int t = 0; t < 8; ++t) {
+            const int c = cbase + 2 * (u0 + t);
+            const int64_t i = i0 + c;
+            if ((u0 + t) < cpr / 2 && i < p.m) {
+              const int64_t idx = i * p.N + jj;
+              S Tt = (S)T[t];
+              if (p.dinv_out) Tt *= (S)p.dinv_out[i];
+              const S out = ka * Tt + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly2);
+              RX[idx] = out;
+              if (p.Wnext) {
+                if constexpr (KIND == 0) {
+                  uint32_t uu;
+                  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(uu) : "f"((float)out));
+                  reinterpret_cast<uint32_t *>(p.Wnext)[idx] = uu;
+                } else {
+                  reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
+                }
+              }
+            }
+          }
+        }
+      }
+      cluster_sync_all();     // nobody leaves while its shared memory may still be read
+    } else
 #pragma unroll 1
     for (int c0 = half * HALF_COLS; c0 < (half + 1) * HALF_COLS; c0 += 32) {
       uint32_t r[32];
@@ -311,8 +381,19 @@ rchfsi_status launch_dense(rchfsi_ctx *h, const CUtensorMap &tmW, const CUtensor
     RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
     attr_set = true;
   }
-  dim3 grid((unsigned)cdiv(p.N, 128), (unsigned)cdiv(p.m, BN));
-  kern<<<grid, 256, Cfg::SMEM_BYTES, h->stream>>>(tmW, tmA, p);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)cdiv(p.N, 128), (unsigned)cdiv(p.m, BN), (unsigned)p.ksplit);
+  cfg.blockDim = dim3(256);
+  cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+  cfg.stream = h->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;     // the K splits of a tile form one cluster
+  attr[0].val.clusterDim.x = 1;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = (unsigned)p.ksplit;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  RCHFSI_CUDA_CHECK(h, cudaLaunchKernelEx(&cfg, kern, tmW, tmA, p));
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }
@@ -362,8 +443,13 @@ rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
     return RCHFSI_ECUDA;
   }
   const CUtensorMap tmW = *ptW, tmA = *ptA;
+  const int32_t nkb = (int32_t)cdiv(h->m, (bf16 ? 64 : 32) * 2);
+  int ks = 1;
+  if (const char *e = getenv("RCHFSI_DENSE_KS")) ks = atoi(e);     // tuning knob
+  if (ks != 1 && ks != 2 && ks != 4 && ks != 8) ks = 1;
+  while (ks > 1 && (nkb < 2 * ks || bn % (2 * ks) != 0)) ks /= 2;
   DenseTcParams p{s.k, s.RY, s.RX, s.G, s.LY, s.chfsi ? h->dinv : nullptr, s.Wnext, h->m, h->N,
-                  (int32_t)cdiv(h->m, (bf16 ? 64 : 32) * 2), getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0};
+                  nkb, ks, getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0};
   if (s.store_prec == RCHFSI_FP64)
     return bf16 ? launch_dense_bn<1, double>(h, bn, tmW, tmA, p) : launch_dense_bn<0, double>(h, bn, tmW, tmA, p);
   return bf16 ? launch_dense_bn<1, float>(h, bn, tmW, tmA, p) : launch_dense_bn<0, float>(h, bn, tmW, tmA, p);

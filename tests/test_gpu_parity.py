@@ -387,3 +387,28 @@ def test_fe_tensor_core_solve_converges_to_exact_eigenvalues():
         np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8, atol=1e-9)
         assert out["resnorm"][:nw].max() <= 1e-8
         sol.close()
+
+
+@pytest.mark.parametrize("bn,ks", [(256, 4), (128, 2)])
+def test_dense_split_k_cluster_fixup_matches_unsplit(monkeypatch, bn, ks):
+    """The optional split-K variant of the dense tcgen05 step (K splits = one thread-block cluster, partial
+    tiles summed over distributed shared memory in fixed rank order) gives the same filtered block as the
+    default unsplit kernel up to FP32 summation order."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(1000, seed=77)
+    N, p = 264, 4
+    outs = []
+    for env in ({}, {"RCHFSI_DENSE_BN": str(bn), "RCHFSI_DENSE_KS": str(ks)}):
+        for k in ("RCHFSI_DENSE_BN", "RCHFSI_DENSE_KS"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        solver, (A, B, Dinv), X, ritz, G = _setup(prob, N, 13, apply_prec="tf32")
+        ev, top = _bounds(prob, A, B)
+        b = (ev[0] - 1e-3, ev[N], top * 1.01)
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+        outs.append(Xd.cpu().numpy())
+        solver.close()
+    assert rel_fro(outs[1], outs[0]) < 1e-5
