@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   const int lane = threadIdx.x & 31;
   const int j0 = blockIdx.x * 128;
   const int64_t cell = p.cell_order[blockIdx.y];
-  const int npanels = (p.ksteps * KSTEP + KR - 1) / KR;
+  const int npanels = (p.debug_mode & 512) ? 0 : (p.ksteps * KSTEP + KR - 1) / KR;   // bit 9: fixed-cost probe
   const uint32_t tmem_cols = (p.np <= 32) ? 32u : (p.np <= 64 ? 64u : (p.np <= 128 ? 128u : (p.np <= 256 ? 256u : 512u)));
 
   for (int t = threadIdx.x; t < p.n_loc; t += blockDim.x)
@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   if (warp == FE_WORK_WARPS && lane == 0) {
     tma_prefetch_desc(&tmA);
     for (int s = 0; s < FE_STAGES; ++s) {
-      mbar_init(full_bar + s, FE_WORK_WARPS + 1);   // 16 gather warps + the TMA expect_tx arrive
+      mbar_init(full_bar + s, FE_WORK_WARPS * 32 + 1);   // every gather thread (async, on landing) + the TMA expect_tx arrive
       mbar_init(empty_bar + s, 1);
     }
     mbar_init(accum_bar, 1);
@@ -156,19 +156,8 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
       const int tid = threadIdx.x;                      // 0 .. 511
       const uint8_t *Wb = reinterpret_cast<const uint8_t *>(p.W);
       constexpr int EB = KIND == 0 ? 4 : 2;             // operand element bytes
-      auto arrive_panel = [&](int pn) {
-        fence_proxy_async();                            // cp.async (generic proxy) data -> tensor-core reads
-        __syncwarp();
-        if (lane == 0) mbar_arrive(full_bar + (pn % FE_STAGES));
-      };
       for (int pn = 0; pn < npanels; ++pn) {
         const int s = pn % FE_STAGES;
-        // publish panel pn-2 BEFORE blocking on the slot of panel pn: otherwise the full barrier of
-        // pn-2 would wait for the MMAs of pn-3 to COMPLETE and every panel would pay a barrier round trip
-        if (pn >= FE_STAGES - 1) {
-          cp_async_wait<FE_STAGES - 2>();
-          arrive_panel(pn - (FE_STAGES - 1));
-        }
         mbar_wait(empty_bar + s, ((pn / FE_STAGES) & 1) ^ 1);
         uint8_t *ws = smem + s * stage_bytes;
 #pragma unroll
@@ -196,10 +185,12 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
           // panel layout [column tile][m][128]: the rows of one tile are 128 * EB bytes apart
           cp_async16(ws + dst_off, Wb + ((uint64_t)rowp * 128 + (ok ? cl : 0)) * EB, ok ? 16u : 0u);
         }
-        cp_async_commit();
+        // the full barrier gets this thread's arrival when its copies have landed: no thread blocks on
+        // its own loads, so all FE_STAGES panels are genuinely in flight
+        cp_async_arrive_noinc(full_bar + s);
       }
+      cp_async_commit();      // keep the epilogue's group accounting clean
       cp_async_wait<0>();
-      for (int pn = max(0, npanels - (FE_STAGES - 1)); pn < npanels; ++pn) arrive_panel(pn);
     }
 
     // ===== epilogue =====
