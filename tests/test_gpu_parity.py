@@ -411,4 +411,6 @@ def test_dense_split_k_cluster_fixup_matches_unsplit(monkeypatch, bn, ks):
         solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
         outs.append(Xd.cpu().numpy())
         solver.close()
-    assert rel_fro(outs[1], outs[0]) < 1e-5
+    # not bitwise: the FP32 partial sums are added in a different order, and the operand shadow of the next
+    # step is rounded to TF32 (2^-11), so a last-bit difference can flip a rounding; bound: operand rounding
+    assert rel_fro(outs[1], outs[0]) < 2.0 ** -11
