@@ -106,7 +106,9 @@ typedef struct {
   uint64_t noise_seed;
   int32_t use_cuda_graph;     /* reserved (ignored): the step coefficients are kernel arguments, so a graph
                                  would have to be re-captured per call; measured launch gaps are < 2 us */
-  int32_t reserved;
+  int32_t g_input_f32;        /* nonzero: the G argument of rchfsi_filter points to FP32 values [m][N] (an FP64
+                                 residual block does not fit at config 5, SURVEY 8(d) memory plan); needs
+                                 store_prec FP32; G is then read in place, no copy is made */
 } rchfsi_options;
 
 /* Fill `opt` with the defaults: apply FP64, store FP64, normalize 1, everything else 0. */

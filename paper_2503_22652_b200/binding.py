@@ -29,7 +29,7 @@ class RchfsiOptions(C.Structure):
     _fields_ = [("apply_prec", C.c_int32), ("store_prec", C.c_int32),
                 ("normalize_columns_before_rr", C.c_int32), ("adaptive_bounds", C.c_int32),
                 ("noise_eps", C.c_double), ("noise_seed", C.c_uint64),
-                ("use_cuda_graph", C.c_int32), ("reserved", C.c_int32)]
+                ("use_cuda_graph", C.c_int32), ("g_input_f32", C.c_int32)]
 
 
 # every symbol include/rchfsi.h declares: name -> (restype, argtypes)
@@ -136,7 +136,7 @@ class Rchfsi:
 
     def __init__(self, A, B=None, dinv=None, block_N=1, apply_prec="fp64", store_prec="fp64",
                  normalize_columns_before_rr=True, adaptive_bounds=False, noise_eps=0.0, noise_seed=0,
-                 use_cuda_graph=False, stream=None):
+                 use_cuda_graph=False, g_input_f32=False, stream=None):
         import torch
         self.lib = load_library()
         self._keep = []
@@ -153,6 +153,7 @@ class Rchfsi:
         opt.noise_eps = float(noise_eps)
         opt.noise_seed = int(noise_seed)
         opt.use_cuda_graph = int(use_cuda_graph)
+        opt.g_input_f32 = int(g_input_f32)
         self.opt = opt
         self.m, self.N = int(self.opA.m), int(block_N)
         self.stream = stream if stream is not None else torch.cuda.current_stream()
@@ -190,7 +191,12 @@ class Rchfsi:
         import torch
         self._block(X, "X")
         if G is not None:
-            self._block(G, "G")
+            if self.opt.g_input_f32:
+                _check_dev(G, torch.float32, "G")
+                if tuple(G.shape) != (self.m, self.N):
+                    raise ValueError("G must have shape (%d, %d)" % (self.m, self.N))
+            else:
+                self._block(G, "G")
         if ritz is not None:
             _check_dev(ritz, torch.float64, "ritz")
         st = self.lib.rchfsi_filter(self.h, method, _ptr(X), _ptr(ritz), _ptr(G), degree, lam_min, lam_T, lam_max)

@@ -75,6 +75,7 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const 
   if (o.apply_prec < RCHFSI_FP64 || o.apply_prec > RCHFSI_BF16) { g_create_error = "unknown apply_prec"; return RCHFSI_EINVAL; }
   if (o.store_prec != RCHFSI_FP64 && o.store_prec != RCHFSI_FP32) { g_create_error = "store_prec must be FP64 or FP32"; return RCHFSI_EINVAL; }
   if (o.store_prec == RCHFSI_FP32 && o.apply_prec == RCHFSI_FP64) { g_create_error = "store FP32 needs a reduced apply_prec"; return RCHFSI_EINVAL; }
+  if (o.g_input_f32 && o.store_prec != RCHFSI_FP32) { g_create_error = "g_input_f32 needs store_prec FP32"; return RCHFSI_EINVAL; }
   if (o.noise_eps < 0) { g_create_error = "noise_eps < 0"; return RCHFSI_EINVAL; }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {

@@ -157,7 +157,8 @@ rchfsi_status step_elementwise(rchfsi_ctx *h, int store_prec, int t_prec, int sh
                                const StepArgs &a);
 // dst(store) = alpha * src(FP64) (+ shadow), used for R_Y = (sigma_1/e) G and G copies
 rchfsi_status scale_convert(rchfsi_ctx *h, int store_prec, int shadow_prec, double alpha,
-                            const double *src, void *dst, void *shadow, int64_t m, int32_t N, int64_t pm = 0);
+                            const void *src, void *dst, void *shadow, int64_t m, int32_t N, int64_t pm = 0,
+                            int src_prec = RCHFSI_FP64);
 // CHFSI first step: Y = alpha * (dinv * T - c X)
 rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_prec, double alpha,
                           double c, const void *T, const double *dinv, const double *X, void *Y,
@@ -194,6 +195,7 @@ struct FusedStep {
   void *Wnext;
   int apply_prec, store_prec;
   bool chfsi;           // dinv applied to the output rows instead of the input
+  bool g_rowmajor;      // G is the caller's row-major [m][N] block even though R_X / R_Y use the panel layout
 };
 bool csr_fused_supported(const rchfsi_ctx *h);
 rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s);

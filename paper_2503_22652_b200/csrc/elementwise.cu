@@ -126,9 +126,9 @@ rchfsi_status step_elementwise(rchfsi_ctx *h, int store_prec, int t_prec, int sh
 // mode 3: X   = RY                                            (Alg. 2 result)
 template <int VEC>
 __global__ void __launch_bounds__(256) misc_kernel(int mode, double alpha, double c, const void *T, int t_prec,
-                                                   const double *dinv, const double *LY, const double *src,
+                                                   const double *dinv, const double *LY, const void *src,
                                                    void *dst, int dst_prec, void *shadow, int shadow_prec,
-                                                   int64_t m, int32_t N, int64_t pm) {
+                                                   int64_t m, int32_t N, int64_t pm, int src_prec) {
   // pm != 0: the library-owned blocks (R_X / R_Y / G copy / shadows) are stored in PANEL layout
   // [ceil(N/128)][m][128] (see fe_tc.cu); user blocks (X, G) are always row-major [m][N].
   const int nv = N / VEC;
@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(256) misc_kernel(int mode, double alpha, doubl
     const int64_t lidx = pm ? (((int64_t)(j >> 7) * pm + row) << 7) + (j & 127) : idx;
     Vals<VEC> out;
     if (mode == 0) {
-      Vals<VEC> s = ld_vec<VEC>(src, idx, RCHFSI_FP64);
+      Vals<VEC> s = ld_vec<VEC>(src, idx, src_prec);
 #pragma unroll
       for (int q = 0; q < VEC; ++q) out.v[q] = alpha * s.v[q];
     } else if (mode == 1) {
@@ -165,22 +165,24 @@ __global__ void __launch_bounds__(256) misc_kernel(int mode, double alpha, doubl
 }
 
 static rchfsi_status launch_misc(rchfsi_ctx *h, int mode, double alpha, double c, const void *T, int t_prec,
-                                 const double *dinv, const double *LY, const double *src, void *dst,
-                                 int dst_prec, void *shadow, int shadow_prec, int64_t m, int32_t N, int64_t pm = 0) {
+                                 const double *dinv, const double *LY, const void *src, void *dst,
+                                 int dst_prec, void *shadow, int shadow_prec, int64_t m, int32_t N, int64_t pm = 0,
+                                 int src_prec = RCHFSI_FP64) {
   if (N % 4 == 0)
     misc_kernel<4><<<ew_grid(m * (N / 4)), 256, 0, h->stream>>>(mode, alpha, c, T, t_prec, dinv, LY, src, dst,
-                                                                 dst_prec, shadow, shadow_prec, m, N, pm);
+                                                                 dst_prec, shadow, shadow_prec, m, N, pm, src_prec);
   else
     misc_kernel<1><<<ew_grid(m * N), 256, 0, h->stream>>>(mode, alpha, c, T, t_prec, dinv, LY, src, dst,
-                                                           dst_prec, shadow, shadow_prec, m, N, pm);
+                                                           dst_prec, shadow, shadow_prec, m, N, pm, src_prec);
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }
 
 rchfsi_status scale_convert(rchfsi_ctx *h, int store_prec, int shadow_prec, double alpha,
-                            const double *src, void *dst, void *shadow, int64_t m, int32_t N, int64_t pm) {
+                            const void *src, void *dst, void *shadow, int64_t m, int32_t N, int64_t pm,
+                            int src_prec) {
   return launch_misc(h, 0, alpha, 0.0, nullptr, 0, nullptr, nullptr, src, dst, store_prec, shadow,
-                     shadow_prec, m, N, pm);
+                     shadow_prec, m, N, pm, src_prec);
 }
 rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_prec, double alpha,
                           double c, const void *T, const double *dinv, const double *X, void *Y,

@@ -46,6 +46,7 @@ struct FeTcParams {
   int32_t np;                 // padded local-node extent of the low-precision copy (= nh * nhalf)
   int32_t ksteps;             // MMA K steps: ceil(n_loc / (8 | 16))
   int32_t stages;
+  int32_t g_rowmajor;         // G is the caller's row-major [m][N] block (FP32, used in place)
   int32_t debug_mode;
 };
 
@@ -230,7 +231,10 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
           uint8_t *d = slot + dst_lane + hsel * (RSTEP * SEG);
           cp_async16(d, srcRX + off, valid ? 16u : 0u);
           cp_async16(d + 1024, srcRY + off, (valid && first) ? 16u : 0u);
-          cp_async16(d + 2048, (has_g ? srcG : srcRX) + off, (valid && first && has_g) ? 16u : 0u);
+          // G: panel layout like R_X / R_Y, or the caller's own row-major block (g_rowmajor)
+          const uint64_t offg = p.g_rowmajor ? ((uint64_t)((w & 0x3FFFFFFFu) - (uint32_t)(blockIdx.x * p.m)) * (uint64_t)p.N + j0) * sizeof(S) + col_bytes
+                                             : off;
+          cp_async16(d + 2048, (has_g ? srcG + offg : srcRX + off), (valid && first && has_g) ? 16u : 0u);
         }
       }
       cp_async_commit();

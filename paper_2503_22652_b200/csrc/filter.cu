@@ -62,7 +62,8 @@ rchfsi_status do_step(rchfsi_ctx *h, const Plan &pl, bool chfsi, const StepCoef 
                       const void *RY, void *RX, const void *G, const double *LY, void *Wnext,
                       uint64_t apply_index) {
   if (pl.fused) {
-    FusedStep s{k, W, RY, RX, G, LY, Wnext, h->opt.apply_prec, pl.store, chfsi};
+    FusedStep s{k, W, RY, RX, G, LY, Wnext, h->opt.apply_prec, pl.store, chfsi,
+                /*g_rowmajor=*/pl.panel && h->opt.g_input_f32 && G != nullptr};
     if (pl.fused == 1) return csr_fused_step(h, s);
     if (pl.fused == 2) return dense_tc_step(h, s);
     return fe_tc_step(h, s);
@@ -101,7 +102,13 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   const int32_t N = h->N;
   const size_t el = (size_t)m * N;
   cudaStream_t st = h->stream;
-  const bool need_gs = !chfsi && (pl.store != RCHFSI_FP64 || pl.panel);
+  // FP32 residual block from the caller (g_input_f32): used in place, never copied (config 5 memory plan)
+  const bool gf32 = !chfsi && h->opt.g_input_f32 != 0;
+  if (gf32 && (!G || pl.store != RCHFSI_FP32)) {
+    h->err = "rchfsi_filter: g_input_f32 needs a non-NULL G and store_prec FP32";
+    return RCHFSI_EINVAL;
+  }
+  const bool need_gs = !chfsi && !gf32 && (pl.store != RCHFSI_FP64 || pl.panel);
   const int64_t pm = pl.panel ? m : 0;
   const size_t el_lib = pl.panel ? (size_t)m * (size_t)cdiv(N, 128) * 128 : el;
   RCHFSI_TRY(ensure_filter_workspace(h, pl, degree, need_gs));
@@ -134,7 +141,8 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
     }
     RCHFSI_TRY(lambda_table(h, ritz, N, degree, e, c, sigma1, h->lam_table));
     RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RX, 0, el_lib * prec_bytes(pl.store), st));       // R_X <- 0
-    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, RY, Wcur, m, N, pm));  // R_Y <- (sigma_1/e) G
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, RY, Wcur, m, N, pm,
+                             gf32 ? RCHFSI_FP32 : RCHFSI_FP64));                          // R_Y <- (sigma_1/e) G
     if (need_gs) {
       RCHFSI_TRY(scale_convert(h, pl.store, 0, 1.0, G, h->Gs, nullptr, m, N, pm));
       Gst = h->Gs;

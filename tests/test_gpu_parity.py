@@ -414,3 +414,33 @@ def test_dense_split_k_cluster_fixup_matches_unsplit(monkeypatch, bn, ks):
     # not bitwise: the FP32 partial sums are added in a different order, and the operand shadow of the next
     # step is rounded to TF32 (2^-11), so a last-bit difference can flip a rounding; bound: operand rounding
     assert rel_fro(outs[1], outs[0]) < 2.0 ** -11
+
+
+@pytest.mark.parametrize("kind", ["fe", "csr"])
+def test_fp32_residual_block_input_is_used_in_place(kind):
+    """g_input_f32 (config-5 memory plan: an FP64 G does not fit): the filter with G given in FP32 equals the
+    filter with the FP64 G up to the FP32 rounding of G, on the panel-layout FE path and a row-major path."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    if kind == "fe":
+        prob = workloads.fe_problem(2, q=3, seed=31)
+        lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+        N, prec = 136, "tf32"
+    else:
+        prob = workloads.config3_sparse_laplacian(n=9, n_wanted=10, block=12, degree=6, seed=5)
+        lam_max, N, prec = 12.0, 12, "fp32"
+    solver, (A, B, Dinv), X, ritz, G = _setup(prob, N, 19, apply_prec=prec, store_prec="fp32")
+    b = (ritz[0] - 1.0, ritz[-1] + 1.0, lam_max)
+    Xa = torch.as_tensor(X).cuda()
+    solver.filter(P.METHOD_RCHFSI, Xa, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), 5, *b)
+    solver.close()
+    As, Bs, dinv = P.upload_problem(prob)
+    s2 = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=prec, store_prec="fp32", g_input_f32=True)
+    Xb = torch.as_tensor(X).cuda()
+    s2.filter(P.METHOD_RCHFSI, Xb, torch.as_tensor(ritz).cuda(), torch.as_tensor(G.astype(np.float32)).cuda(), 5, *b)
+    assert rel_fro(Xb.cpu().numpy(), Xa.cpu().numpy()) < 1e-5
+    with pytest.raises(P.RchfsiError):      # G is mandatory in this mode
+        s2.filter(P.METHOD_RCHFSI, Xb, torch.as_tensor(ritz).cuda(), None, 5, *b)
+    s2.close()
+    with pytest.raises(P.RchfsiError):      # and needs FP32 storage
+        P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=prec, store_prec="fp64", g_input_f32=True)
