@@ -34,6 +34,8 @@ WORKLOADS = {
     "c2": dict(name="configs[1] dense generalized m=4000 N=240 p=25, TF32 apply, FP64 recurrence", apply="tf32", store="fp64"),
     "c3": dict(name="configs[2] 64^3 7-point Laplacian CSR m=262144 N=300 p=30, FP32 SpMM, FP64 recurrence", apply="fp32", store="fp64"),
     "c4": dict(name="configs[3] FE 16^3 cells degree 6 m=912673 N=1200 p=40", apply="tf32", store="fp64"),
+    "c5": dict(name="configs[4] FE 24^3 cells degree 6 m=3048625 N=2400 p=50, filter only (FP32 recurrence and residual "
+                    "block, FP64 X; TF32 operands: the BF16 shadow pair does not fit next to them)", apply="tf32", store="fp32"),
 }
 
 
@@ -53,6 +55,13 @@ def make_problem(wl):
     elif wl == "c3":
         p = workloads.config3_sparse_laplacian()
         b = (None, None, p["lam_max"])
+    elif wl == "c5":
+        p = workloads.config5_fe()
+        if FE_CELLS is not None:
+            import workloads.fe as wfe
+            p = wfe.fe_problem(FE_CELLS, 6, 5, cell_dtype=np.float32)
+            p.update(n_wanted=2048, block=2400, degree=50, tol=1e-8, x0_seed=2005)
+        b = (None, None, None)
     elif wl == "c4":
         p = workloads.config4_fe()
         if FE_CELLS is not None:
@@ -149,7 +158,7 @@ def run_reference(args):
     prob, b = make_problem(args.workload)
     N, p = prob["block"], prob["degree"]
     A, B, Dinv = orc.operators_from_workload(prob)
-    max_cols = {"c1": 60, "c2": 48, "c3": 8, "c4": 2}[args.workload]
+    max_cols = {"c1": 60, "c2": 48, "c3": 8, "c4": 2, "c5": 1}[args.workload]
     rng = np.random.default_rng(123)
     X = rng.standard_normal((prob["m"], max_cols))
     ritz = np.sort(rng.uniform(0.0, 1.0, max_cols))
@@ -173,6 +182,76 @@ def run_reference(args):
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def run_c5(args, prob, As, Bs, dinv, dev, wl, apply_prec, store_prec, world, rank):
+    """configs[4] at full size is a memory plan: X FP64 58.5 GB + G FP32 29.3 GB (caller-owned, read in
+    place) + R_X, R_Y FP32 58.5 GB + operator copies.  Only the FILTER is timed: the inputs of Alg. 3 are seeded
+    synthetic blocks generated on the device (a Rayleigh-Ritz at this size needs the chunked variant),
+    and there is no host copy of an 88 GB input set, so no end-to-end number."""
+    import torch
+    import paper_2503_22652_b200 as P
+    m, N, p = prob["m"], prob["block"], prob["degree"]
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(prob.get("x0_seed", 5) + rank)
+    X = torch.empty((m, N), dtype=torch.float64, device=dev)
+    for r0 in range(0, m, 65536):                      # row chunks: no second full-size temporary
+        X[r0:r0 + 65536].normal_(generator=gen)
+    X *= 1.0 / np.sqrt(m)
+    G = torch.empty((m, N), dtype=torch.float32, device=dev)
+    for r0 in range(0, m, 65536):
+        G[r0:r0 + 65536].normal_(generator=gen)
+    G *= 1e-3
+    ritz = torch.linspace(-9.0, 3.0, N, dtype=torch.float64, device=dev)
+    bounds = (-10.0, 3.5, fe_lam_max(prob))
+    solver = P.Rchfsi(As, None, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec, g_input_f32=True)
+    for _ in range(args.warmup):
+        solver.filter(P.METHOD_RCHFSI, X, ritz, G, p, *bounds)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    l0 = solver.launch_count()
+    steps = max(1, min(args.steps, 3))
+    total_ms, step_ms, step_n = 0.0, 0.0, 0
+    for _ in range(steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        solver.filter(P.METHOD_RCHFSI, X, ritz, G, p, *bounds)
+        e1.record()
+        ms_k, n_k = solver.last_filter_step_ms()
+        total_ms += e0.elapsed_time(e1)
+        step_ms += ms_k
+        step_n += n_k
+    launches = solver.launch_count() - l0
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    finite = bool(torch.isfinite(X[::4096]).all().item())
+    from paper_2503_22652_b200.sharding import reduce_job
+    total_ms, updates = reduce_job(total_ms, float(m) * N * p)
+    if rank != 0:
+        return
+    ms_per_step = total_ms / steps
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    sm = step_ms / max(1, step_n)
+    byts = 4.0 * m * N * 4 + prob["n_cells"] * prob["n_loc"] ** 2 * 4.0
+    gbs = byts / (sm * 1e-3) / 1e9
+    out = {"metric": METRIC, "value": updates / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps,
+           "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "tf32", "data": "synthetic",
+           "config": {"workload": wl["name"], "m": m, "block_N": N, "degree": p, "apply_prec": apply_prec,
+                      "store_prec": store_prec, "l2": "inputs (176 GB) far larger than L2",
+                      "device_bytes_allocated": int(torch.cuda.memory_allocated()), "output_finite": finite},
+           "clocks": sampler.summary(), "gpu_launches": int(launches),
+           "e2e": None, "e2e_note": "no host copy of the 88 GB input set exists on this box",
+           "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                        "traffic": None, "kernel": "fused FE operator + recurrence step (8 colour launches)",
+                        "step_launch_ms": sm, "peak_source": "measured" if peaks else "fallback"}}
+    print(json.dumps(out))
 
 
 def main():
@@ -218,7 +297,13 @@ def main():
     m, N, p, nw = prob["m"], prob["block"], prob["degree"], prob["n_wanted"]
     As, Bs, dinv = P.upload_problem(prob, device=dev)
     noise = dict(noise_eps=prob.get("noise_eps", 0.0), noise_seed=1234) if args.workload == "c1" else {}
-    solver = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec, **noise)
+    solver = None
+    if args.workload != "c5":
+        solver = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec, **noise)
+
+    if args.workload == "c5":
+        run_c5(args, prob, As, Bs, dinv, dev, wl, apply_prec, store_prec, world, rank)
+        return
 
     # inputs of Alg. 3: B-orthonormal X, Ritz values and G from one Rayleigh-Ritz on a seeded block
     X0 = prob.get("X0")
@@ -363,7 +448,7 @@ def main():
 
     if not args.no_cpu_baseline:
         Xc, rc, Gc = X.cpu().numpy(), rz, G.cpu().numpy()
-        max_cols = {"c1": 60, "c2": 240, "c3": 16, "c4": 2}[args.workload]
+        max_cols = {"c1": 60, "c2": 240, "c3": 16, "c4": 2, "c5": 1}[args.workload]
         v, nc, dt = oracle_filter_time(prob, Xc, rc, Gc, p, bounds, max_cols)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
                                "sample": "oracle.filter_rchfsi, %d of %d columns, full m and degree, %.1f s" % (nc, N, dt)}
