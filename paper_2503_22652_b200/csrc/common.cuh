@@ -80,6 +80,9 @@ struct rchfsi_ctx {
 
   // Rayleigh-Ritz workspace
   double *rr1 = nullptr, *rr2 = nullptr, *rr3 = nullptr;   // [m][N] FP64
+  double *rrc1 = nullptr, *rrc2 = nullptr, *rrp = nullptr; // chunked variant: [m][cw] x 2, [rp][N]
+  int32_t rr_cw = 0; int64_t rr_rp = 0;
+  float *Gsolve32 = nullptr;                               // [m][N] FP32 residual block of rchfsi_solve (chunked mode)
   double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
@@ -134,7 +137,7 @@ inline size_t prec_bytes(int prec) {
 // For FE the output is accumulated with atomics into a zeroed T.
 template <typename TC>
 rchfsi_status op_apply_simt(rchfsi_ctx *h, const rchfsi_operator &op, const double *dinv_in,
-                            const TC *W, TC *T, int32_t N);
+                            const TC *W, TC *T, int32_t N, int64_t ldw = 0, int64_t ldt = 0);
 
 // Lambda_k table, k = 0..p (eq. (12)): table[k][j].
 rchfsi_status lambda_table(rchfsi_ctx *h, const double *ritz, int32_t N, int32_t p, double e,
@@ -180,6 +183,9 @@ rchfsi_status add_column_noise(rchfsi_ctx *h, int t_prec, void *T, int64_t m, in
 // G = AX - BX diag(ritz), res_j = ||G_j||
 rchfsi_status residual_block(rchfsi_ctx *h, const double *AX, const double *BX, const double *ritz,
                              double *G, double *res, int64_t m, int32_t N);
+rchfsi_status residual_window(rchfsi_ctx *h, const double *AX, int64_t lda, const double *BX, int64_t ldb,
+                              const double *ritz, void *G, int64_t ldg, int g_prec, double *res2, int64_t m, int32_t w);
+rchfsi_status sqrt_inplace(rchfsi_ctx *h, double *v, int32_t N);
 rchfsi_status symmetrize(rchfsi_ctx *h, double *H, int32_t N);
 rchfsi_status fe_check_symmetric(rchfsi_ctx *h, const rchfsi_operator &op, double *max_asym_host);
 
@@ -207,5 +213,10 @@ rchfsi_status fe_tc_step(rchfsi_ctx *h, const FusedStep &s);
 // ---- rr.cu -----------------------------------------------------------------------------
 rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, double *G_out,
                                  double *res_out);
+// Memory-light variant (SURVEY 8(d) config-5 plan): Gram matrices over column chunks, rotation by row panels in
+// place, residual block recomputed per column chunk and written in g_prec (FP64 or FP32).
+rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, void *G_out, int g_prec,
+                                    double *res_out);
+bool rr_wants_chunked(rchfsi_ctx *h);
 
 }  // namespace rchfsi

@@ -285,6 +285,36 @@ __global__ void __launch_bounds__(256) residual_kernel(const double *AX, const d
     if (res2) atomicAdd(res2 + j, s);
   }
 }
+// column-window variant for the chunked Rayleigh-Ritz: AX, BX, G have their own row pitches and G may be FP32
+__global__ void __launch_bounds__(256) residual_window_kernel(const double *AX, int64_t lda, const double *BX, int64_t ldb,
+                                                              const double *ritz, void *G, int64_t ldg, int g_prec,
+                                                              double *res2, int64_t m, int32_t w, int64_t rows_per_cta) {
+  const int64_t r0 = blockIdx.x * rows_per_cta;
+  const int64_t r1 = min(m, r0 + rows_per_cta);
+  for (int j = threadIdx.x; j < w; j += blockDim.x) {
+    const double lam = ritz[j];
+    double s = 0.0;
+    for (int64_t i = r0; i < r1; ++i) {
+      const double g = AX[i * lda + j] - BX[i * ldb + j] * lam;
+      if (G) {
+        if (g_prec == RCHFSI_FP32) reinterpret_cast<float *>(G)[i * ldg + j] = (float)g;
+        else reinterpret_cast<double *>(G)[i * ldg + j] = g;
+      }
+      s += g * g;
+    }
+    if (res2) atomicAdd(res2 + j, s);
+  }
+}
+rchfsi_status residual_window(rchfsi_ctx *h, const double *AX, int64_t lda, const double *BX, int64_t ldb,
+                              const double *ritz, void *G, int64_t ldg, int g_prec, double *res2, int64_t m, int32_t w) {
+  int64_t ctas = std::min<int64_t>(m, 148 * 8);
+  int64_t rows = cdiv(m, ctas);
+  ctas = cdiv(m, rows);
+  residual_window_kernel<<<(unsigned)ctas, 256, 0, h->stream>>>(AX, lda, BX, ldb, ritz, G, ldg, g_prec, res2, m, w, rows);
+  LAUNCH_CHECK(h);
+  return RCHFSI_OK;
+}
+rchfsi_status sqrt_inplace(rchfsi_ctx *h, double *v, int32_t N);
 __global__ void sqrt_kernel(double *v, int32_t N) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j < N) v[j] = sqrt(v[j]);
@@ -302,6 +332,12 @@ rchfsi_status residual_block(rchfsi_ctx *h, const double *AX, const double *BX, 
     sqrt_kernel<<<(unsigned)cdiv(N, 128), 128, 0, h->stream>>>(res, N);
     LAUNCH_CHECK(h);
   }
+  return RCHFSI_OK;
+}
+
+rchfsi_status sqrt_inplace(rchfsi_ctx *h, double *v, int32_t N) {
+  sqrt_kernel<<<(unsigned)cdiv(N, 128), 128, 0, h->stream>>>(v, N);
+  LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }
 

@@ -60,10 +60,10 @@ rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t deg
 // One operator apply + recurrence update, fused when a fused kernel exists for this plan.
 rchfsi_status do_step(rchfsi_ctx *h, const Plan &pl, bool chfsi, const StepCoef &k, const void *W,
                       const void *RY, void *RX, const void *G, const double *LY, void *Wnext,
-                      uint64_t apply_index) {
+                      uint64_t apply_index, bool g_rowmajor = false) {
   if (pl.fused) {
     FusedStep s{k, W, RY, RX, G, LY, Wnext, h->opt.apply_prec, pl.store, chfsi,
-                /*g_rowmajor=*/pl.panel && h->opt.g_input_f32 && G != nullptr};
+                /*g_rowmajor=*/pl.panel && g_rowmajor && G != nullptr};
     if (pl.fused == 1) return csr_fused_step(h, s);
     if (pl.fused == 2) return dense_tc_step(h, s);
     return fe_tc_step(h, s);
@@ -82,10 +82,11 @@ rchfsi_status do_step(rchfsi_ctx *h, const Plan &pl, bool chfsi, const StepCoef 
 
 }  // namespace
 
-extern "C" {
-
-rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const double *ritz, const double *G,
-                            int32_t degree, double lam_min, double lam_T, double lam_max) {
+// G_arg points to FP64 values, or to FP32 values when g_is_f32 (caller's g_input_f32 option, or the FP32
+// residual block rchfsi_solve keeps in its memory-light mode)
+static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, const double *ritz, const void *G_arg,
+                                 bool g_is_f32, int32_t degree, double lam_min, double lam_T, double lam_max) {
+  const double *G = reinterpret_cast<const double *>(G_arg);
   if (!h) return RCHFSI_EINVAL;
   if (!X || (reinterpret_cast<uintptr_t>(X) & 15u)) { h->err = "rchfsi_filter: X null or misaligned"; return RCHFSI_EINVAL; }
   if (method != RCHFSI_METHOD_CHFSI && method != RCHFSI_METHOD_RCHFSI) { h->err = "rchfsi_filter: unknown method"; return RCHFSI_EINVAL; }
@@ -103,7 +104,7 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   const size_t el = (size_t)m * N;
   cudaStream_t st = h->stream;
   // FP32 residual block from the caller (g_input_f32): used in place, never copied (config 5 memory plan)
-  const bool gf32 = !chfsi && h->opt.g_input_f32 != 0;
+  const bool gf32 = !chfsi && g_is_f32;
   if (gf32 && (!G || pl.store != RCHFSI_FP32)) {
     h->err = "rchfsi_filter: g_input_f32 needs a non-NULL G and store_prec FP32";
     return RCHFSI_EINVAL;
@@ -177,7 +178,7 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
     StepCoef kc{2.0 * sigma2 / e, -2.0 * sigma2 * c / e, -sigma * sigma2};
     const double *LY = chfsi ? nullptr : h->lam_table + (size_t)(k - 1) * N;
     const void *W = pl.shadow ? Wcur : RY;
-    RCHFSI_TRY(do_step(h, pl, chfsi, kc, W, RY, RX, chfsi ? nullptr : Gst, LY, Wnext, apply_index++));
+    RCHFSI_TRY(do_step(h, pl, chfsi, kc, W, RY, RX, chfsi ? nullptr : Gst, LY, Wnext, apply_index++, gf32));
     std::swap(RX, RY);                       // swap(R_X, R_Y)
     if (pl.shadow) std::swap(Wcur, Wnext);
     sigma = sigma2;
@@ -190,6 +191,14 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   else
     RCHFSI_TRY(finish_block(h, pl.store, RY, nullptr, nullptr, X, m, N, pm));
   return RCHFSI_OK;
+}
+
+extern "C" {
+
+rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const double *ritz, const double *G,
+                            int32_t degree, double lam_min, double lam_T, double lam_max) {
+  if (!h) return RCHFSI_EINVAL;
+  return filter_impl(h, method, X, ritz, G, h->opt.g_input_f32 != 0, degree, lam_min, lam_T, lam_max);
 }
 
 rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host, const double *ritz_host,
@@ -223,10 +232,27 @@ rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n
   const size_t el = (size_t)h->m * N;
   cudaStream_t st = h->stream;
   const bool rch = (method == RCHFSI_METHOD_RCHFSI);
-  if (rch && !h->Gtmp) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gtmp, el * 8));
+  // Memory-light mode when three more FP64 blocks do not fit (config 5): chunked Rayleigh-Ritz, and with FP32
+  // recurrence storage the residual block G is kept in FP32 (SURVEY 8(d) memory plan) and read in place.
+  const bool chunked = rr_wants_chunked(h);
+  const bool g32 = chunked && rch && h->opt.store_prec == RCHFSI_FP32;
+  void *Gbuf = nullptr;
+  if (rch) {
+    if (g32) {
+      if (!h->Gsolve32) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gsolve32, el * 4));
+      Gbuf = h->Gsolve32;
+    } else {
+      if (!h->Gtmp) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gtmp, el * 8));
+      Gbuf = h->Gtmp;
+    }
+  }
+  auto do_rr = [&]() -> rchfsi_status {
+    if (chunked) return rayleigh_ritz_chunked(h, X, h->ritz_dev, Gbuf, g32 ? RCHFSI_FP32 : RCHFSI_FP64, h->res_dev);
+    return rayleigh_ritz_impl(h, X, h->ritz_dev, (double *)Gbuf, h->res_dev);
+  };
   std::vector<double> ritz(N), res(N);
   // reading S2: one Rayleigh-Ritz on the initial guess gives B-orthonormal X, Lambda and G
-  RCHFSI_TRY(rayleigh_ritz_impl(h, X, h->ritz_dev, rch ? h->Gtmp : nullptr, h->res_dev));
+  RCHFSI_TRY(do_rr());
   rchfsi_status result = RCHFSI_ENOTCONVERGED;
   int32_t it = 0;
   for (it = 1; it <= max_iter; ++it) {
@@ -235,8 +261,8 @@ rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n
       RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
       if (ritz[0] < ritz[N - 1] && ritz[N - 1] < lam_max) { lam_min = ritz[0]; lam_T = ritz[N - 1]; }
     }
-    RCHFSI_TRY(rchfsi_filter(h, method, X, h->ritz_dev, rch ? h->Gtmp : nullptr, degree, lam_min, lam_T, lam_max));
-    RCHFSI_TRY(rayleigh_ritz_impl(h, X, h->ritz_dev, rch ? h->Gtmp : nullptr, h->res_dev));
+    RCHFSI_TRY(filter_impl(h, method, X, h->ritz_dev, Gbuf, g32, degree, lam_min, lam_T, lam_max));
+    RCHFSI_TRY(do_rr());
     RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(res.data(), h->res_dev, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
     RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
     double worst = 0.0;

@@ -11,7 +11,7 @@ template <typename TC>
 __global__ void __launch_bounds__(256) dense_apply_kernel(const double *__restrict__ A, int64_t lda,
                                                           const double *__restrict__ dinv,
                                                           const TC *__restrict__ W, TC *__restrict__ T,
-                                                          int64_t m, int32_t N) {
+                                                          int64_t m, int32_t N, int64_t ldw, int64_t ldt) {
   constexpr int BM = 64, BN = 64, BK = 16;
   __shared__ TC As[BK][BM + 4];
   __shared__ TC Ws[BK][BN + 4];
@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(256) dense_apply_kernel(const double *__restri
       int j = j0 + c;
       TC v = TC(0);
       if (k < m && j < N) {
-        v = W[k * (int64_t)N + j];
+        v = W[k * ldw + j];
         if (dinv) v = (TC)dinv[k] * v;
       }
       Ws[kk][c] = v;
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(256) dense_apply_kernel(const double *__restri
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
       int j = j0 + tx * 4 + c;
-      if (j < N) T[i * (int64_t)N + j] = acc[r][c];
+      if (j < N) T[i * ldt + j] = acc[r][c];
     }
   }
 }
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(256) csr_apply_kernel(const int64_t *__restric
                                                         const double *__restrict__ vals,
                                                         const double *__restrict__ dinv,
                                                         const TC *__restrict__ W, TC *__restrict__ T,
-                                                        int64_t m, int32_t N) {
+                                                        int64_t m, int32_t N, int64_t ldw, int64_t ldt) {
   const int nvec = N / VEC;
   const int64_t total = m * nvec;
   for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
@@ -98,11 +98,11 @@ __global__ void __launch_bounds__(256) csr_apply_kernel(const int64_t *__restric
       double a = vals[t];
       if (dinv) a *= dinv[col];
       const TC av = (TC)a;
-      const TC *w = W + (int64_t)col * N + (int64_t)v * VEC;
+      const TC *w = W + (int64_t)col * ldw + (int64_t)v * VEC;
 #pragma unroll
       for (int q = 0; q < VEC; ++q) acc[q] += av * w[q];
     }
-    TC *o = T + row * (int64_t)N + (int64_t)v * VEC;
+    TC *o = T + row * ldt + (int64_t)v * VEC;
 #pragma unroll
     for (int q = 0; q < VEC; ++q) o[q] = acc[q];
   }
@@ -116,7 +116,7 @@ template <typename TC, typename TM, int CT>
 __global__ void fe_apply_kernel(const TM *__restrict__ cell_mats, int64_t cell_stride,
                                 const int32_t *__restrict__ conn, int32_t n_loc,
                                 const double *__restrict__ dinv, const TC *__restrict__ W,
-                                TC *__restrict__ T, int32_t N) {
+                                TC *__restrict__ T, int32_t N, int64_t ldw, int64_t ldt) {
   extern __shared__ __align__(16) unsigned char fe_smem[];
   TC *Ws = reinterpret_cast<TC *>(fe_smem);              // [n_loc][CT]
   const int64_t cell = blockIdx.y;
@@ -128,7 +128,7 @@ __global__ void fe_apply_kernel(const TM *__restrict__ cell_mats, int64_t cell_s
     int64_t row = cn[b];
     TC v = TC(0);
     if (j < N) {
-      v = W[row * N + j];
+      v = W[row * ldw + j];
       if (dinv) v = (TC)dinv[row] * v;
     }
     Ws[e] = v;
@@ -145,7 +145,7 @@ __global__ void fe_apply_kernel(const TM *__restrict__ cell_mats, int64_t cell_s
 #pragma unroll
       for (int c = 0; c < CT; ++c) acc[c] += av * w[c];
     }
-    TC *o = T + (int64_t)cn[a] * N + j0;
+    TC *o = T + (int64_t)cn[a] * ldt + j0;
 #pragma unroll
     for (int c = 0; c < CT; ++c)
       if (j0 + c < N) atomicAdd(o + c, acc[c]);
@@ -154,28 +154,36 @@ __global__ void fe_apply_kernel(const TM *__restrict__ cell_mats, int64_t cell_s
 
 template <typename TC>
 rchfsi_status op_apply_simt(rchfsi_ctx *h, const rchfsi_operator &op, const double *dinv_in,
-                            const TC *W, TC *T, int32_t N) {
+                            const TC *W, TC *T, int32_t N, int64_t ldw, int64_t ldt) {
+  // N columns of a block whose rows are ldw (input) / ldt (output) elements apart: a column window of a
+  // wider block is W + first_column with ldw = the block's width (0 = contiguous, ld = N)
   cudaStream_t st = h->stream;
   const int64_t m = op.m;
+  if (ldw == 0) ldw = N;
+  if (ldt == 0) ldt = N;
   if (op.kind == RCHFSI_OP_DENSE) {
     dim3 grid((unsigned)cdiv(N, 64), (unsigned)cdiv(m, 64));
-    dense_apply_kernel<TC><<<grid, 256, 0, st>>>(op.dense, op.lda, dinv_in, W, T, m, N);
+    dense_apply_kernel<TC><<<grid, 256, 0, st>>>(op.dense, op.lda, dinv_in, W, T, m, N, ldw, ldt);
     LAUNCH_CHECK(h);
   } else if (op.kind == RCHFSI_OP_CSR) {
     constexpr int V = (sizeof(TC) == 8) ? 2 : 4;
-    if (N % V == 0) {
+    if (N % V == 0 && ldw % V == 0 && ldt % V == 0 && (reinterpret_cast<uintptr_t>(W) & 15u) == 0 &&
+        (reinterpret_cast<uintptr_t>(T) & 15u) == 0) {
       int64_t total = m * (N / V);
       unsigned grid = (unsigned)std::min<int64_t>(cdiv(total, 256), 148 * 64);
-      csr_apply_kernel<TC, V><<<grid, 256, 0, st>>>(op.rowptr, op.colind, op.vals, dinv_in, W, T, m, N);
+      csr_apply_kernel<TC, V><<<grid, 256, 0, st>>>(op.rowptr, op.colind, op.vals, dinv_in, W, T, m, N, ldw, ldt);
     } else {
       int64_t total = m * N;
       unsigned grid = (unsigned)std::min<int64_t>(cdiv(total, 256), 148 * 64);
-      csr_apply_kernel<TC, 1><<<grid, 256, 0, st>>>(op.rowptr, op.colind, op.vals, dinv_in, W, T, m, N);
+      csr_apply_kernel<TC, 1><<<grid, 256, 0, st>>>(op.rowptr, op.colind, op.vals, dinv_in, W, T, m, N, ldw, ldt);
     }
     LAUNCH_CHECK(h);
   } else if (op.kind == RCHFSI_OP_FE) {
     constexpr int CT = (sizeof(TC) == 8) ? 12 : 24;
-    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(T, 0, sizeof(TC) * (size_t)m * N, st));
+    if (ldt == N)
+      RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(T, 0, sizeof(TC) * (size_t)m * N, st));
+    else
+      RCHFSI_CUDA_CHECK(h, cudaMemset2DAsync(T, sizeof(TC) * (size_t)ldt, 0, sizeof(TC) * (size_t)N, (size_t)m, st));
     dim3 grid((unsigned)cdiv(N, CT), (unsigned)op.n_cells);
     int threads = (int)std::min<int64_t>(1024, cdiv(op.n_loc, 32) * 32);
     size_t smem = sizeof(TC) * (size_t)op.n_loc * CT;
@@ -183,11 +191,11 @@ rchfsi_status op_apply_simt(rchfsi_ctx *h, const rchfsi_operator &op, const doub
     if (op.cell_mats) {
       auto kern = fe_apply_kernel<TC, double, CT>;
       RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      kern<<<grid, threads, smem, st>>>(op.cell_mats, stride, op.conn, op.n_loc, dinv_in, W, T, N);
+      kern<<<grid, threads, smem, st>>>(op.cell_mats, stride, op.conn, op.n_loc, dinv_in, W, T, N, ldw, ldt);
     } else {
       auto kern = fe_apply_kernel<TC, float, CT>;
       RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      kern<<<grid, threads, smem, st>>>(op.cell_mats_f32, stride, op.conn, op.n_loc, dinv_in, W, T, N);
+      kern<<<grid, threads, smem, st>>>(op.cell_mats_f32, stride, op.conn, op.n_loc, dinv_in, W, T, N, ldw, ldt);
     }
     LAUNCH_CHECK(h);
   } else {
@@ -197,8 +205,8 @@ rchfsi_status op_apply_simt(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   return RCHFSI_OK;
 }
 template rchfsi_status op_apply_simt<double>(rchfsi_ctx *, const rchfsi_operator &, const double *,
-                                             const double *, double *, int32_t);
+                                             const double *, double *, int32_t, int64_t, int64_t);
 template rchfsi_status op_apply_simt<float>(rchfsi_ctx *, const rchfsi_operator &, const double *,
-                                            const float *, float *, int32_t);
+                                            const float *, float *, int32_t, int64_t, int64_t);
 
 }  // namespace rchfsi

@@ -2,6 +2,7 @@
 // Off the hot path: the Gram and rotation products are plain library
 // GEMMs (cuBLAS dgemm) and the N x N generalized eigenproblem is cuSOLVER dsygvd; the operator
 // applies are this library's FP64 kernels.
+#include <cstdlib>
 #include "common.cuh"
 
 namespace rchfsi {
@@ -23,7 +24,7 @@ namespace rchfsi {
     }                                                                             \
   } while (0)
 
-static rchfsi_status ensure_rr_workspace(rchfsi_ctx *h) {
+static rchfsi_status ensure_rr_workspace(rchfsi_ctx *h, bool full_blocks = true) {
   const size_t blk = sizeof(double) * (size_t)h->m * h->N;
   const size_t nn = sizeof(double) * (size_t)h->N * h->N;
   if (!h->cublas) {
@@ -35,9 +36,11 @@ static rchfsi_status ensure_rr_workspace(rchfsi_ctx *h) {
     CUSOLVER_CHECK(h, cusolverDnCreate(&h->cusolver));
     CUSOLVER_CHECK(h, cusolverDnSetStream(h->cusolver, h->stream));
   }
-  if (!h->rr1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr1, blk));
-  if (!h->rr3) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr3, blk));
-  if (h->B.present && !h->rr2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr2, blk));
+  if (full_blocks) {
+    if (!h->rr1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr1, blk));
+    if (!h->rr3) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr3, blk));
+    if (h->B.present && !h->rr2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr2, blk));
+  }
   if (!h->Ha) RCHFSI_TRY(dev_alloc(h, (void **)&h->Ha, nn));
   if (!h->Hb) RCHFSI_TRY(dev_alloc(h, (void **)&h->Hb, nn));
   if (!h->ritz_dev) RCHFSI_TRY(dev_alloc(h, (void **)&h->ritz_dev, sizeof(double) * h->N));
@@ -124,6 +127,107 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
       BX = h->rr1;
     }
     RCHFSI_TRY(residual_block(h, T3, BX, h->ritz_dev, G_out, res_out, m, N));
+  }
+  if (ritz_out && ritz_out != h->ritz_dev)
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz_out, h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));
+  return RCHFSI_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Chunked variant: no full-size temporary.  Extra device memory: two [m][cw] FP64 chunks and one [rp][N]
+// FP64 row panel (about 6 GB + 3 GB at config 5 instead of 3 x 58.5 GB).
+bool rr_wants_chunked(rchfsi_ctx *h) {
+  if (const char *e = getenv("RCHFSI_RR_CHUNKED")) return atoi(e) != 0;      // test / tuning knob
+  if (h->rrc1) return true;                                                    // decided earlier for this handle
+  if (h->rr1) return false;                                                    // full workspace already there
+  size_t free_b = 0, total_b = 0;
+  if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return false;
+  const size_t blk = sizeof(double) * (size_t)h->m * h->N;
+  return free_b < (size_t)(3.3 * (double)blk);
+}
+
+rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, void *G_out, int g_prec,
+                                    double *res_out) {
+  RCHFSI_TRY(ensure_rr_workspace(h, false));
+  const int64_t m = h->m;
+  const int32_t N = h->N;
+  cudaStream_t st = h->stream;
+  if (!h->rrc1) {
+    int64_t cw = (int64_t)(6.0e9 / (16.0 * (double)m));
+    cw = std::max<int64_t>(8, std::min<int64_t>(N, cw / 8 * 8));
+    int64_t rp = (int64_t)(3.0e9 / (8.0 * (double)N));
+    rp = std::max<int64_t>(256, std::min<int64_t>(m, rp));
+    h->rr_cw = (int32_t)cw;
+    h->rr_rp = rp;
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)m * cw));
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc2, sizeof(double) * (size_t)m * cw));
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)rp * N));
+  }
+  const int32_t cw = h->rr_cw;
+  const double one = 1.0, zero = 0.0;
+  if (h->opt.normalize_columns_before_rr) {
+    RCHFSI_TRY(column_sumsq(h, RCHFSI_FP64, Y, m, N, h->colnorm));
+    RCHFSI_TRY(scale_columns_inv_norm(h, Y, m, N, h->colnorm));
+  }
+  // Gram matrices, one column chunk of A Y / B Y at a time:  H[:, c0:c0+w] = Y^T (Op Y[:, c0:c0+w])
+  for (int32_t c0 = 0; c0 < N; c0 += cw) {
+    const int32_t w = std::min(cw, N - c0);
+    RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, Y + c0, h->rrc1, w, N, w));
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N, w, (int)m, &one, Y, N, h->rrc1, w, &zero,
+                                h->Ha + (size_t)c0 * N, N));
+    if (h->B.present) {
+      RCHFSI_TRY(op_apply_simt<double>(h, h->B.d, nullptr, Y + c0, h->rrc2, w, N, w));
+      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N, w, (int)m, &one, Y, N, h->rrc2, w, &zero,
+                                  h->Hb + (size_t)c0 * N, N));
+    } else {
+      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N, w, (int)m, &one, Y, N, Y + c0, N, &zero,
+                                  h->Hb + (size_t)c0 * N, N));
+    }
+    h->launches += 2;
+  }
+  RCHFSI_TRY(symmetrize(h, h->Ha, N));
+  RCHFSI_TRY(symmetrize(h, h->Hb, N));
+  CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
+                                     CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,
+                                     h->sy_lwork, h->sy_info));
+  h->launches++;
+  int info = 0;
+  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(&info, h->sy_info, sizeof(int), cudaMemcpyDeviceToHost, st));
+  RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
+  if (info != 0) {
+    h->err = "Rayleigh-Ritz: dsygvd info = " + std::to_string(info) +
+             (info > N ? " (Y^T B Y not positive definite)" : " (eigensolver did not converge)");
+    return RCHFSI_EBREAKDOWN;
+  }
+  const double *E = h->Ha;
+  // X = Y E in place, one row panel at a time (row-major rows r0.. are the columns r0.. of the N x m view)
+  for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
+    const int64_t rows = std::min<int64_t>(h->rr_rp, m - r0);
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_T, CUBLAS_OP_N, N, (int)rows, N, &one, E, N, Y + (size_t)r0 * N, N,
+                                &zero, h->rrp, N));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y + (size_t)r0 * N, h->rrp, sizeof(double) * (size_t)rows * N,
+                                         cudaMemcpyDeviceToDevice, st));
+    h->launches++;
+  }
+  if (G_out || res_out) {
+    // G = A X - B X Lambda recomputed from the rotated block, chunk by chunk (two more operator applies instead
+    // of two more full-size temporaries)
+    if (res_out) RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(res_out, 0, sizeof(double) * N, st));
+    const size_t gel = (g_prec == RCHFSI_FP32) ? sizeof(float) : sizeof(double);
+    for (int32_t c0 = 0; c0 < N; c0 += cw) {
+      const int32_t w = std::min(cw, N - c0);
+      RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, Y + c0, h->rrc1, w, N, w));
+      const double *BX = Y + c0;
+      int64_t ldb = N;
+      if (h->B.present) {
+        RCHFSI_TRY(op_apply_simt<double>(h, h->B.d, nullptr, Y + c0, h->rrc2, w, N, w));
+        BX = h->rrc2;
+        ldb = w;
+      }
+      void *Gc = G_out ? (void *)(reinterpret_cast<uint8_t *>(G_out) + (size_t)c0 * gel) : nullptr;
+      RCHFSI_TRY(residual_window(h, h->rrc1, w, BX, ldb, h->ritz_dev + c0, Gc, N, g_prec, res_out ? res_out + c0 : nullptr, m, w));
+    }
+    if (res_out) RCHFSI_TRY(sqrt_inplace(h, res_out, N));
   }
   if (ritz_out && ritz_out != h->ritz_dev)
     RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz_out, h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));

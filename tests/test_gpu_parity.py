@@ -444,3 +444,52 @@ def test_fp32_residual_block_input_is_used_in_place(kind):
     s2.close()
     with pytest.raises(P.RchfsiError):      # and needs FP32 storage
         P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=prec, store_prec="fp64", g_input_f32=True)
+
+
+def test_chunked_rayleigh_ritz_matches_oracle_and_full_variant(monkeypatch):
+    """Memory-light Rayleigh-Ritz (Gram matrices over column chunks, in-place row-panel rotation, residual block
+    recomputed per chunk; SURVEY 8(d) config-5 plan), forced with RCHFSI_RR_CHUNKED=1: same Ritz values,
+    B-orthonormal X, G and residual norms as the oracle."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_RR_CHUNKED", "1")
+    for prob, N in ((small_dense_generalized(300, seed=3), 24), (workloads.fe_problem(2, q=3, seed=8), 20)):
+        A, B, Dinv = oracle_ops(prob)
+        m = prob["m"]
+        Y = np.random.default_rng(8).standard_normal((m, N)) * np.logspace(0, 4, N)[None, :]
+        ritz_o, X_o, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, Y)
+        res_o = orc.residual_norms(AX, BX, ritz_o)
+        As, Bs, dinv = P.upload_problem(prob)
+        s = P.Rchfsi(As, Bs, dinv, block_N=N)
+        ritz, X, G, res = s.rayleigh_ritz(torch.as_tensor(Y).cuda())
+        np.testing.assert_allclose(ritz.cpu().numpy(), ritz_o, rtol=1e-10, atol=1e-10)
+        Xg = X.cpu().numpy()
+        BXg = B.apply(Xg)
+        np.testing.assert_allclose(Xg.T @ BXg, np.eye(N), rtol=0, atol=1e-9)
+        Gref = A.apply(Xg) - BXg * ritz.cpu().numpy()[None, :]
+        np.testing.assert_allclose(G.cpu().numpy(), Gref, rtol=0, atol=1e-9 * max(1.0, np.abs(Gref).max()))
+        np.testing.assert_allclose(res.cpu().numpy(), res_o, rtol=1e-5, atol=1e-9)
+        s.close()
+
+
+def test_memory_light_solve_keeps_fp32_residual_block(monkeypatch):
+    """rchfsi_solve in the memory-light mode (chunked Rayleigh-Ritz + FP32 G read in place by the fused steps):
+    still converges to the exact eigenvalues with residual <= 1e-8."""
+    torch = _torch()
+    import scipy.linalg as sla
+    import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_RR_CHUNKED", "1")
+    prob = workloads.fe_problem(2, q=4, seed=11)
+    A, B, Dinv = oracle_ops(prob)
+    m = prob["m"]
+    ev = sla.eigh(A.apply(np.eye(m)), B.apply(np.eye(m)), eigvals_only=True)
+    lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    N, nw, p = 16, 8, 30
+    X0 = np.random.default_rng(2).standard_normal((m, N))
+    As, Bs, dinv = P.upload_problem(prob)
+    sol = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec="tf32", store_prec="fp32", adaptive_bounds=True)
+    out = sol.solve(P.METHOD_RCHFSI, torch.as_tensor(X0).cuda(), nw, p, ev[0] - 1.0, ev[N], lam_max, tol=1e-8, max_iter=80)
+    assert out["converged"], out["history"][-5:]
+    np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8, atol=1e-9)
+    assert out["resnorm"][:nw].max() <= 1e-8
+    sol.close()
