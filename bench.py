@@ -283,6 +283,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--solve", action="store_true", help="also run rchfsi_solve on c4 (about a minute)")
+    ap.add_argument("--solve-method", default="rchfsi", choices=["rchfsi", "chfsi"],
+                    help="method of the extra solve (chfsi = Algorithm 2 with the same kernels, the paper's comparator)")
+    ap.add_argument("--solve-iters", type=int, default=60)
     ap.add_argument("--fe-cells", type=int, default=None, help="c4 only: cells per direction (profiling a smaller mesh)")
     ap.add_argument("--block", type=int, default=None, help="override the block width N (profiling)")
     args = ap.parse_args()
@@ -458,9 +461,11 @@ def main():
         so = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec,
                       adaptive_bounds=(args.workload != "c1"), **noise)
         t0 = time.perf_counter()
-        r = so.solve(P.METHOD_RCHFSI, Xs, nw, p, lam_min, lam_T, lam_max, tol=1e-8, max_iter=60)
-        out["solve"] = {"final_residual": float(r["resnorm"][:nw].max()), "iters": int(r["iters"]),
-                        "converged": bool(r["converged"]), "seconds": time.perf_counter() - t0}
+        meth = P.METHOD_RCHFSI if args.solve_method == "rchfsi" else P.METHOD_CHFSI
+        r = so.solve(meth, Xs, nw, p, lam_min, lam_T, lam_max, tol=1e-8, max_iter=args.solve_iters)
+        out["solve"] = {"method": args.solve_method, "final_residual": float(r["resnorm"][:nw].max()),
+                        "iters": int(r["iters"]), "converged": bool(r["converged"]),
+                        "seconds": time.perf_counter() - t0, "history": [float(x) for x in r["history"]]}
         so.close()
 
     if not args.no_cpu_baseline:

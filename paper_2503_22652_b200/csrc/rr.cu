@@ -154,7 +154,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   cudaStream_t st = h->stream;
   if (!h->rrc1) {
     int64_t cw = (int64_t)(6.0e9 / (16.0 * (double)m));
-    cw = std::max<int64_t>(8, std::min<int64_t>(N, cw / 8 * 8));
+    cw = std::max<int64_t>(8, std::min<int64_t>(N, cw >= 48 ? cw / 48 * 48 : cw / 8 * 8));   // multiples of the FE column tile
     int64_t rp = (int64_t)(3.0e9 / (8.0 * (double)N));
     rp = std::max<int64_t>(256, std::min<int64_t>(m, rp));
     h->rr_cw = (int32_t)cw;
