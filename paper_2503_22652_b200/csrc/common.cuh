@@ -83,6 +83,9 @@ struct rchfsi_ctx {
   double *rrc1 = nullptr, *rrc2 = nullptr, *rrp = nullptr; // chunked variant: [m][cw] x 2, [rp][N]
   int32_t rr_cw = 0; int64_t rr_rp = 0;
   float *Gsolve32 = nullptr;                               // [m][N] FP32 residual block of rchfsi_solve (chunked mode)
+  double *feg_W = nullptr, *feg_T = nullptr, *feg_A = nullptr;  // fe_rr.cu scratch: gathered operand, product, FP64 cell batch
+  const double **feg_ptrs = nullptr;                        // [3][feg_ptr_cap] pointer arrays of the batched GEMM
+  size_t feg_w_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0;
   double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
@@ -209,6 +212,13 @@ bool dense_tc_supported(const rchfsi_ctx *h);
 rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s);
 bool fe_tc_supported(const rchfsi_ctx *h);
 rchfsi_status fe_tc_step(rchfsi_ctx *h, const FusedStep &s);
+
+// ---- fe_rr.cu / fe_tc.cu ---------------------------------------------------------------
+rchfsi_status fe_ensure_coloring(rchfsi_ctx *h);
+bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op);
+// T = Op W in FP64 through gather -> batched DGEMM -> coloured scatter (Rayleigh-Ritz only)
+rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,
+                            int64_t ldw = 0, int64_t ldt = 0);
 
 // ---- rr.cu -----------------------------------------------------------------------------
 rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, double *G_out,

@@ -1,0 +1,139 @@
+// FP64 FE operator apply for the Rayleigh-Ritz (off the hot path):
+//   T = sum_c P_c^T A_c P_c W     (PAPER.md:357 Remark 4.1, in FP64 with the exact cell matrices)
+// as  gather -> batched library DGEMM -> scatter, one colour of the cell colouring at a time.  Cells of one
+// colour share no node, so the scatter is a plain read-modify-write (deterministic, no atomics); the first
+// colour that touches a node writes, the later ones add (same first-touch flags as the tensor-core filter).
+// The filter's own FP64 mode keeps the hand-written kernel of kernels_simt.cu; this path only serves
+// rchfsi_rayleigh_ritz / rchfsi_solve, where the products are plain library GEMMs like the Gram and rotation
+// products next to them.  Measured at config 4: 158 -> see DESIGN.md section 8.
+#include <algorithm>
+#include <cstdlib>
+#include "common.cuh"
+
+namespace rchfsi {
+
+namespace {
+
+// Wg[bi][b][j] = W[conn[cell(bi)][b]][j]
+__global__ void feg_gather_kernel(const double *__restrict__ W, int64_t ldw, const int32_t *__restrict__ conn,
+                                  const int32_t *__restrict__ cells, int32_t n_loc, int32_t N, double *__restrict__ Wg,
+                                  int64_t rows) {
+  const int64_t total = rows * N;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = t / N;
+    const int j = (int)(t - r * N);
+    const int64_t bi = r / n_loc;
+    const int b = (int)(r - bi * n_loc);
+    const int64_t row = conn[(int64_t)cells[bi] * n_loc + b];
+    Wg[t] = W[row * ldw + j];
+  }
+}
+
+// T[conn[cell(bi)][a]][j] (= | +=) Tc[bi][a][j]
+__global__ void feg_scatter_kernel(const double *__restrict__ Tc, const int32_t *__restrict__ conn,
+                                   const uint8_t *__restrict__ flags, const int32_t *__restrict__ cells, int32_t n_loc,
+                                   int32_t N, double *__restrict__ T, int64_t ldt, int64_t rows) {
+  const int64_t total = rows * N;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = t / N;
+    const int j = (int)(t - r * N);
+    const int64_t bi = r / n_loc;
+    const int a = (int)(r - bi * n_loc);
+    const int64_t e = (int64_t)cells[bi] * n_loc + a;
+    double *o = T + (int64_t)conn[e] * ldt + j;
+    const double v = Tc[t];
+    *o = (flags[e] & 1) ? v : *o + v;
+  }
+}
+
+__global__ void feg_convert_kernel(const float *__restrict__ mats, const int32_t *__restrict__ cells, int64_t per,
+                                   double *__restrict__ out, int64_t batch, int shared) {
+  const int64_t total = batch * per;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t bi = t / per;
+    out[t] = (double)mats[(shared ? 0 : (int64_t)cells[bi]) * per + (t - bi * per)];
+  }
+}
+
+// pointer arrays of the batched GEMM: [0] = gathered operand, [1] = cell matrix, [2] = product
+__global__ void feg_pointers_kernel(const double **ptrs, int64_t batch, int64_t cap, const double *Wg, double *Tc,
+                                    int64_t wstride, const double *mats, int64_t mstride, const int32_t *cells,
+                                    const double *conv) {
+  const int64_t bi = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (bi >= batch) return;
+  ptrs[bi] = Wg + bi * wstride;
+  ptrs[cap + bi] = conv ? conv + bi * mstride : mats + (int64_t)cells[bi] * mstride;
+  ptrs[2 * cap + bi] = Tc + bi * wstride;
+}
+
+}  // namespace
+
+bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op) {
+  if (getenv("RCHFSI_RR_FE_SIMT")) return false;                       // A/B knob: keep the hand-written kernel
+  const rchfsi_operator &A = h->A.d;
+  return op.kind == RCHFSI_OP_FE && A.kind == RCHFSI_OP_FE && op.conn == A.conn && op.n_cells == A.n_cells &&
+         op.n_loc == A.n_loc && h->cublas != nullptr && (op.cell_mats != nullptr || op.cell_mats_f32 != nullptr);
+}
+
+rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,
+                            int64_t ldw, int64_t ldt) {
+  if (ldw == 0) ldw = N;
+  if (ldt == 0) ldt = N;
+  RCHFSI_TRY(fe_ensure_coloring(h));
+  const FeColoring &col = h->coloring;
+  const int32_t nl = op.n_loc;
+  const bool conv = (op.cell_mats == nullptr);
+  const int64_t mper = op.cell_shared ? 0 : (int64_t)nl * nl;
+  // scratch: gathered operand + product (+ FP64 copy of FP32 cell matrices), about 1.5 GB
+  const size_t per_cell = 2 * sizeof(double) * (size_t)nl * N + (conv ? sizeof(double) * (size_t)nl * nl : 0);
+  int64_t max_color = 0;
+  for (int k = 0; k < col.n_colors; ++k) max_color = std::max(max_color, col.color_begin[k + 1] - col.color_begin[k]);
+  const int64_t cap = std::max<int64_t>(1, std::min<int64_t>(max_color, (int64_t)(1.5e9 / (double)per_cell)));
+  const size_t need_w = sizeof(double) * (size_t)cap * nl * N;
+  if (h->feg_w_bytes < need_w) {
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_W, need_w));
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_T, need_w));
+    h->feg_w_bytes = need_w;
+  }
+  if (conv && h->feg_a_cells < cap) {
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_A, sizeof(double) * (size_t)cap * nl * nl));
+    h->feg_a_cells = cap;
+  }
+  if (h->feg_ptr_cap < cap) {
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_ptrs, sizeof(double *) * 3 * (size_t)cap));
+    h->feg_ptr_cap = cap;
+  }
+  const int64_t pcap = h->feg_ptr_cap;
+  const double one = 1.0, zero = 0.0;
+  cudaStream_t st = h->stream;
+  const unsigned ew = 148 * 16;
+  for (int k = 0; k < col.n_colors; ++k)
+    for (int64_t b0 = col.color_begin[k]; b0 < col.color_begin[k + 1]; b0 += cap) {
+      const int64_t batch = std::min<int64_t>(cap, col.color_begin[k + 1] - b0);
+      const int32_t *cells = col.cell_order + b0;
+      const int64_t rows = batch * nl;
+      feg_gather_kernel<<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows);
+      LAUNCH_CHECK(h);
+      if (conv) {
+        feg_convert_kernel<<<ew, 256, 0, st>>>(op.cell_mats_f32, cells, (int64_t)nl * nl, h->feg_A, op.cell_shared ? 1 : batch, op.cell_shared ? 1 : 0);
+        LAUNCH_CHECK(h);
+      }
+      feg_pointers_kernel<<<(unsigned)cdiv(batch, 128), 128, 0, st>>>(h->feg_ptrs, batch, pcap, h->feg_W, h->feg_T, (int64_t)nl * N,
+                                                                      op.cell_mats, mper, cells, conv ? h->feg_A : nullptr);
+      LAUNCH_CHECK(h);
+      // row-major [nl][N] blocks are column-major N x nl: Tc (N x nl) = Wg (N x nl) * Acm (nl x nl), where the
+      // column-major read of the row-major cell matrix is Acm(b, a) = A_c[a][b], so Tc[a][j] = sum_b A_c[a][b] Wg[b][j]
+      cublasStatus_t cs = cublasDgemmBatched(h->cublas, CUBLAS_OP_N, CUBLAS_OP_N, N, nl, nl, &one, h->feg_ptrs, N,
+                                             h->feg_ptrs + pcap, nl, &zero, (double **)(h->feg_ptrs + 2 * pcap), N, (int)batch);
+      if (cs != CUBLAS_STATUS_SUCCESS) {
+        h->err = "cublasDgemmBatched (FE apply): status " + std::to_string((int)cs);
+        return RCHFSI_ECUDA;
+      }
+      h->launches++;
+      feg_scatter_kernel<<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows);
+      LAUNCH_CHECK(h);
+    }
+  return RCHFSI_OK;
+}
+
+}  // namespace rchfsi

@@ -2,6 +2,7 @@
 // Off the hot path: the Gram and rotation products are plain library
 // GEMMs (cuBLAS dgemm) and the N x N generalized eigenproblem is cuSOLVER dsygvd; the operator
 // applies are this library's FP64 kernels.
+#include <cstdio>
 #include <cstdlib>
 #include "common.cuh"
 
@@ -24,6 +25,35 @@ namespace rchfsi {
     }                                                                             \
   } while (0)
 
+// RCHFSI_RR_TIMING=1: synchronise after each phase and print its wall time to stderr (diagnostic only).
+struct PhaseTimer {
+  rchfsi_ctx *h;
+  bool on;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  explicit PhaseTimer(rchfsi_ctx *hh) : h(hh), on(getenv("RCHFSI_RR_TIMING") != nullptr) {
+    if (on) {
+      cudaEventCreate(&e0);
+      cudaEventCreate(&e1);
+      cudaEventRecord(e0, h->stream);
+    }
+  }
+  void lap(const char *what) {
+    if (!on) return;
+    cudaEventRecord(e1, h->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    fprintf(stderr, "[rchfsi rr] %-28s %10.3f ms\n", what, ms);
+    cudaEventRecord(e0, h->stream);
+  }
+  ~PhaseTimer() {
+    if (on) {
+      cudaEventDestroy(e0);
+      cudaEventDestroy(e1);
+    }
+  }
+};
+
 static rchfsi_status ensure_rr_workspace(rchfsi_ctx *h, bool full_blocks = true) {
   const size_t blk = sizeof(double) * (size_t)h->m * h->N;
   const size_t nn = sizeof(double) * (size_t)h->N * h->N;
@@ -41,8 +71,14 @@ static rchfsi_status ensure_rr_workspace(rchfsi_ctx *h, bool full_blocks = true)
     if (!h->rr3) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr3, blk));
     if (h->B.present && !h->rr2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr2, blk));
   }
-  if (!h->Ha) RCHFSI_TRY(dev_alloc(h, (void **)&h->Ha, nn));
-  if (!h->Hb) RCHFSI_TRY(dev_alloc(h, (void **)&h->Hb, nn));
+  if (!h->Ha) {   // only the lower triangles are ever formed: keep the never-read upper parts defined
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->Ha, nn));
+    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(h->Ha, 0, nn, h->stream));
+  }
+  if (!h->Hb) {
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->Hb, nn));
+    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(h->Hb, 0, nn, h->stream));
+  }
   if (!h->ritz_dev) RCHFSI_TRY(dev_alloc(h, (void **)&h->ritz_dev, sizeof(double) * h->N));
   if (!h->res_dev) RCHFSI_TRY(dev_alloc(h, (void **)&h->res_dev, sizeof(double) * h->N));
   if (!h->colnorm) RCHFSI_TRY(dev_alloc(h, (void **)&h->colnorm, sizeof(double) * 2 * h->N));
@@ -58,14 +94,37 @@ static rchfsi_status ensure_rr_workspace(rchfsi_ctx *h, bool full_blocks = true)
   return RCHFSI_OK;
 }
 
+// FP64 operator apply of the Rayleigh-Ritz: FE operators go through the batched-GEMM path of fe_rr.cu when it
+// applies (3-4x the hand-written FP64 kernel at config 4), everything else through kernels_simt.cu.
+static rchfsi_status apply64(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,
+                             int64_t ldw = 0, int64_t ldt = 0) {
+  if (fe_apply_gemm_supported(h, op)) return fe_apply_gemm(h, op, W, T, N, ldw, ldt);
+  return op_apply_simt<double>(h, op, nullptr, W, T, N, ldw, ldt);
+}
+
+// flops of one operator apply on an N-column block (to choose between re-applying and rotating, below)
+static double apply_flops(const rchfsi_operator &op, int32_t N) {
+  if (op.kind == RCHFSI_OP_DENSE) return 2.0 * (double)op.m * (double)op.m * N;
+  if (op.kind == RCHFSI_OP_CSR) return 2.0 * (double)op.nnz * N;
+  return 2.0 * (double)op.n_cells * (double)op.n_loc * (double)op.n_loc * N;
+}
+
 // Row-major [m][N] blocks are column-major N x m matrices with leading dimension N.
 // Gram: H = U^T V  (N x N).  In the column-major view Uc (N x m): Uc * Vc^T has entry
 // (i,j) = sum_r U[r][i] V[r][j], stored column-major = H^T row-major; H is symmetrised after.
+// Only the lower triangle (column-major i >= j) is formed, in slabs of GRAM_SLAB columns: U^T V is symmetric up
+// to rounding for V = Op U with a symmetric operator, and dsygvd reads the lower triangle only.  Slab [c0, c0+w)
+// needs the rows i >= c0, so the work is a little over half of the full product.
+constexpr int32_t GRAM_SLAB = 256;
 static rchfsi_status gram(rchfsi_ctx *h, const double *U, const double *V, double *H) {
   const double one = 1.0, zero = 0.0;
-  CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, h->N, h->N, (int)h->m, &one, U, h->N, V,
-                              h->N, &zero, H, h->N));
-  h->launches++;
+  const int32_t N = h->N;
+  for (int32_t c0 = 0; c0 < N; c0 += GRAM_SLAB) {
+    const int32_t w = std::min(GRAM_SLAB, N - c0);
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)h->m, &one, U + c0, N, V + c0, N,
+                                &zero, H + (size_t)c0 * N + c0, N));
+    h->launches++;
+  }
   return RCHFSI_OK;
 }
 // Out[r][j] = sum_l In[r][l] E[l][j], E column-major N x N (cuSOLVER layout):
@@ -84,21 +143,24 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
   const int32_t N = h->N;
   const size_t blk = sizeof(double) * (size_t)m * N;
   cudaStream_t st = h->stream;
+  PhaseTimer pt(h);
   if (h->opt.normalize_columns_before_rr) {   // reading S6
     RCHFSI_TRY(column_sumsq(h, RCHFSI_FP64, Y, m, N, h->colnorm));
     RCHFSI_TRY(scale_columns_inv_norm(h, Y, m, N, h->colnorm));
   }
+  pt.lap("normalise columns");
   double *AY = h->rr1;
-  RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, Y, AY, N));
+  RCHFSI_TRY(apply64(h, h->A.d, Y, AY, N));
+  pt.lap("A Y");
   const double *BY = Y;
   if (h->B.present) {
-    RCHFSI_TRY(op_apply_simt<double>(h, h->B.d, nullptr, Y, h->rr2, N));
+    RCHFSI_TRY(apply64(h, h->B.d, Y, h->rr2, N));
     BY = h->rr2;
   }
+  pt.lap("B Y");
   RCHFSI_TRY(gram(h, Y, AY, h->Ha));
   RCHFSI_TRY(gram(h, Y, BY, h->Hb));
-  RCHFSI_TRY(symmetrize(h, h->Ha, N));
-  RCHFSI_TRY(symmetrize(h, h->Hb, N));
+  pt.lap("Gram x2 (dgemm, lower)");
   // H_a E = H_b E Lambda, E^T H_b E = I, ascending (LAPACK dsygv type 1)
   CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
                                      CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,
@@ -112,21 +174,29 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
              (info > N ? " (Y^T B Y not positive definite)" : " (eigensolver did not converge)");
     return RCHFSI_EBREAKDOWN;
   }
+  pt.lap("dsygvd");
   const double *E = h->Ha;   // eigenvectors overwrite H_a, column-major
   double *T3 = h->rr3;
   // X = Y E
   RCHFSI_TRY(rotate(h, Y, E, T3));
   RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y, T3, blk, cudaMemcpyDeviceToDevice, st));
+  pt.lap("X = Y E (dgemm + copy)");
   const bool need_res = (G_out != nullptr) || (res_out != nullptr);
   if (need_res) {
-    // AX = (AY) E -> T3 ; BX = (BY) E -> rr1 (AY is dead by then) or X itself when B = I
-    RCHFSI_TRY(rotate(h, AY, E, T3));
+    // AX and BX: either rotate the products already at hand, AX = (AY) E, BX = (BY) E (2 m N^2 flops each), or
+    // apply the operators to the rotated block again -- whichever is less work (sparse / FE operators: re-apply)
     const double *BX = Y;
+    const double rot_flops = 2.0 * (double)m * (double)N * (double)N;
+    if (apply_flops(h->A.d, N) < rot_flops) RCHFSI_TRY(apply64(h, h->A.d, Y, T3, N));
+    else RCHFSI_TRY(rotate(h, AY, E, T3));
     if (h->B.present) {
-      RCHFSI_TRY(rotate(h, h->rr2, E, h->rr1));
+      if (apply_flops(h->B.d, N) < rot_flops) RCHFSI_TRY(apply64(h, h->B.d, Y, h->rr1, N));
+      else RCHFSI_TRY(rotate(h, h->rr2, E, h->rr1));   // AY is dead by then
       BX = h->rr1;
     }
+    pt.lap("AX, BX (re-apply or rotate)");
     RCHFSI_TRY(residual_block(h, T3, BX, h->ritz_dev, G_out, res_out, m, N));
+    pt.lap("residual block");
   }
   if (ritz_out && ritz_out != h->ritz_dev)
     RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz_out, h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));
@@ -172,21 +242,20 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   // Gram matrices, one column chunk of A Y / B Y at a time:  H[:, c0:c0+w] = Y^T (Op Y[:, c0:c0+w])
   for (int32_t c0 = 0; c0 < N; c0 += cw) {
     const int32_t w = std::min(cw, N - c0);
-    RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, Y + c0, h->rrc1, w, N, w));
-    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N, w, (int)m, &one, Y, N, h->rrc1, w, &zero,
-                                h->Ha + (size_t)c0 * N, N));
+    // lower triangle only (rows i >= c0 of this column slab): dsygvd reads nothing else
+    RCHFSI_TRY(apply64(h, h->A.d, Y + c0, h->rrc1, w, N, w));
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc1, w, &zero,
+                                h->Ha + (size_t)c0 * N + c0, N));
     if (h->B.present) {
-      RCHFSI_TRY(op_apply_simt<double>(h, h->B.d, nullptr, Y + c0, h->rrc2, w, N, w));
-      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N, w, (int)m, &one, Y, N, h->rrc2, w, &zero,
-                                  h->Hb + (size_t)c0 * N, N));
+      RCHFSI_TRY(apply64(h, h->B.d, Y + c0, h->rrc2, w, N, w));
+      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc2, w, &zero,
+                                  h->Hb + (size_t)c0 * N + c0, N));
     } else {
-      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N, w, (int)m, &one, Y, N, Y + c0, N, &zero,
-                                  h->Hb + (size_t)c0 * N, N));
+      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, Y + c0, N, &zero,
+                                  h->Hb + (size_t)c0 * N + c0, N));
     }
     h->launches += 2;
   }
-  RCHFSI_TRY(symmetrize(h, h->Ha, N));
-  RCHFSI_TRY(symmetrize(h, h->Hb, N));
   CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
                                      CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,
                                      h->sy_lwork, h->sy_info));
@@ -216,11 +285,11 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     const size_t gel = (g_prec == RCHFSI_FP32) ? sizeof(float) : sizeof(double);
     for (int32_t c0 = 0; c0 < N; c0 += cw) {
       const int32_t w = std::min(cw, N - c0);
-      RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, Y + c0, h->rrc1, w, N, w));
+      RCHFSI_TRY(apply64(h, h->A.d, Y + c0, h->rrc1, w, N, w));
       const double *BX = Y + c0;
       int64_t ldb = N;
       if (h->B.present) {
-        RCHFSI_TRY(op_apply_simt<double>(h, h->B.d, nullptr, Y + c0, h->rrc2, w, N, w));
+        RCHFSI_TRY(apply64(h, h->B.d, Y + c0, h->rrc2, w, N, w));
         BX = h->rrc2;
         ldb = w;
       }

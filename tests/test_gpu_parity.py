@@ -493,3 +493,43 @@ def test_memory_light_solve_keeps_fp32_residual_block(monkeypatch):
     np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8, atol=1e-9)
     assert out["resnorm"][:nw].max() <= 1e-8
     sol.close()
+
+
+@pytest.mark.parametrize("f32_cells", [False, True])
+@pytest.mark.parametrize("chunked", ["0", "1"])
+def test_fe_rayleigh_ritz_batched_gemm_apply_equals_handwritten_apply(monkeypatch, f32_cells, chunked):
+    """The Rayleigh-Ritz applies FE operators through gather -> batched DGEMM -> coloured scatter (fe_rr.cu);
+    RCHFSI_RR_FE_SIMT=1 keeps the hand-written FP64 kernel.  Both must give the oracle's Ritz values, a
+    B-orthonormal X and the exact residual block, with FP64 or FP32-only cell matrices (config-5 storage), in the
+    full and in the chunked variant (lower-triangle Gram matrices in both)."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_RR_CHUNKED", chunked)
+    prob = dict(workloads.fe_problem(3, q=3, seed=5))
+    if f32_cells:   # the operator IS the FP32-rounded one: give the oracle the same numbers
+        prob["A_cells"] = prob["A_cells"].astype(np.float32).astype(np.float64)
+    N = 28
+    A, B, Dinv = oracle_ops(prob)
+    m = prob["m"]
+    Y = np.random.default_rng(21).standard_normal((m, N)) * np.logspace(0, 3, N)[None, :]
+    ritz_o, X_o, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, Y)
+    res_o = orc.residual_norms(AX, BX, ritz_o)
+    out = {}
+    for simt in (False, True):
+        if simt:
+            monkeypatch.setenv("RCHFSI_RR_FE_SIMT", "1")
+        else:
+            monkeypatch.delenv("RCHFSI_RR_FE_SIMT", raising=False)
+        As, Bs, dinv = P.upload_problem(prob, fe_cells_f32_only=f32_cells)
+        s = P.Rchfsi(As, Bs, dinv, block_N=N)
+        ritz, X, G, res = s.rayleigh_ritz(torch.as_tensor(Y).cuda())
+        out[simt] = (ritz.cpu().numpy(), X.cpu().numpy(), G.cpu().numpy(), res.cpu().numpy())
+        s.close()
+        np.testing.assert_allclose(out[simt][0], ritz_o, rtol=1e-10, atol=1e-10)
+        Xg = out[simt][1]
+        BXg = B.apply(Xg)
+        np.testing.assert_allclose(Xg.T @ BXg, np.eye(N), rtol=0, atol=1e-9)
+        Gref = A.apply(Xg) - BXg * out[simt][0][None, :]
+        np.testing.assert_allclose(out[simt][2], Gref, rtol=0, atol=1e-9 * max(1.0, np.abs(Gref).max()))
+        np.testing.assert_allclose(out[simt][3], res_o, rtol=1e-5, atol=1e-9)
+    np.testing.assert_allclose(out[False][0], out[True][0], rtol=1e-12, atol=1e-12)
