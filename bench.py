@@ -261,7 +261,7 @@ def run_c5(args, prob, As, Bs, dinv, dev, wl, apply_prec, store_prec, world, ran
             X[r0:r0 + 65536].normal_(generator=gen)
         so = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec=store_prec, adaptive_bounds=True)
         t0 = time.perf_counter()
-        r = so.solve(P.METHOD_RCHFSI, X, prob["n_wanted"], p, -100.0, 0.0, bounds[2], tol=1e-8, max_iter=60)
+        r = so.solve(P.METHOD_RCHFSI, X, prob["n_wanted"], p, -100.0, 0.0, bounds[2], tol=1e-8, max_iter=args.solve_iters)
         out["solve"] = {"final_residual": float(r["resnorm"][:prob["n_wanted"]].max()), "iters": int(r["iters"]),
                         "converged": bool(r["converged"]), "seconds": time.perf_counter() - t0,
                         "history": [float(x) for x in r["history"]],

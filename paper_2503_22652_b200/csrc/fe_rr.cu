@@ -14,35 +14,54 @@ namespace rchfsi {
 
 namespace {
 
+// One warp per gathered row, lanes along the contiguous columns (16-byte accesses when VEC = 2).
 // Wg[bi][b][j] = W[conn[cell(bi)][b]][j]
+template <int VEC>
 __global__ void feg_gather_kernel(const double *__restrict__ W, int64_t ldw, const int32_t *__restrict__ conn,
                                   const int32_t *__restrict__ cells, int32_t n_loc, int32_t N, double *__restrict__ Wg,
-                                  int64_t rows) {
-  const int64_t total = rows * N;
-  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t r = t / N;
-    const int j = (int)(t - r * N);
-    const int64_t bi = r / n_loc;
-    const int b = (int)(r - bi * n_loc);
-    const int64_t row = conn[(int64_t)cells[bi] * n_loc + b];
-    Wg[t] = W[row * ldw + j];
+                                  int32_t rows) {
+  const int lane = threadIdx.x & 31;
+  const int wpb = blockDim.x >> 5;
+  for (int32_t r = blockIdx.x * wpb + (threadIdx.x >> 5); r < rows; r += gridDim.x * wpb) {
+    const int32_t bi = r / n_loc;
+    const int32_t b = r - bi * n_loc;
+    const double *src = W + (int64_t)conn[(int64_t)cells[bi] * n_loc + b] * ldw;
+    double *dst = Wg + (int64_t)r * N;
+    if constexpr (VEC == 2) {
+      for (int j = lane; j < N / 2; j += 32) reinterpret_cast<double2 *>(dst)[j] = reinterpret_cast<const double2 *>(src)[j];
+    } else {
+      for (int j = lane; j < N; j += 32) dst[j] = src[j];
+    }
   }
 }
 
 // T[conn[cell(bi)][a]][j] (= | +=) Tc[bi][a][j]
+template <int VEC>
 __global__ void feg_scatter_kernel(const double *__restrict__ Tc, const int32_t *__restrict__ conn,
                                    const uint8_t *__restrict__ flags, const int32_t *__restrict__ cells, int32_t n_loc,
-                                   int32_t N, double *__restrict__ T, int64_t ldt, int64_t rows) {
-  const int64_t total = rows * N;
-  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t r = t / N;
-    const int j = (int)(t - r * N);
-    const int64_t bi = r / n_loc;
-    const int a = (int)(r - bi * n_loc);
+                                   int32_t N, double *__restrict__ T, int64_t ldt, int32_t rows) {
+  const int lane = threadIdx.x & 31;
+  const int wpb = blockDim.x >> 5;
+  for (int32_t r = blockIdx.x * wpb + (threadIdx.x >> 5); r < rows; r += gridDim.x * wpb) {
+    const int32_t bi = r / n_loc;
+    const int32_t a = r - bi * n_loc;
     const int64_t e = (int64_t)cells[bi] * n_loc + a;
-    double *o = T + (int64_t)conn[e] * ldt + j;
-    const double v = Tc[t];
-    *o = (flags[e] & 1) ? v : *o + v;
+    double *o = T + (int64_t)conn[e] * ldt;
+    const double *src = Tc + (int64_t)r * N;
+    const bool first = flags[e] & 1;
+    if constexpr (VEC == 2) {
+      for (int j = lane; j < N / 2; j += 32) {
+        double2 v = reinterpret_cast<const double2 *>(src)[j];
+        if (!first) {
+          const double2 old = reinterpret_cast<double2 *>(o)[j];
+          v.x += old.x;
+          v.y += old.y;
+        }
+        reinterpret_cast<double2 *>(o)[j] = v;
+      }
+    } else {
+      for (int j = lane; j < N; j += 32) o[j] = first ? src[j] : o[j] + src[j];
+    }
   }
 }
 
@@ -88,7 +107,7 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   const size_t per_cell = 2 * sizeof(double) * (size_t)nl * N + (conv ? sizeof(double) * (size_t)nl * nl : 0);
   int64_t max_color = 0;
   for (int k = 0; k < col.n_colors; ++k) max_color = std::max(max_color, col.color_begin[k + 1] - col.color_begin[k]);
-  const int64_t cap = std::max<int64_t>(1, std::min<int64_t>(max_color, (int64_t)(1.5e9 / (double)per_cell)));
+  const int64_t cap = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(max_color, (int64_t)(1.5e9 / (double)per_cell)), ((int64_t)1 << 30) / nl));
   const size_t need_w = sizeof(double) * (size_t)cap * nl * N;
   if (h->feg_w_bytes < need_w) {
     RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_W, need_w));
@@ -104,6 +123,8 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
     h->feg_ptr_cap = cap;
   }
   const int64_t pcap = h->feg_ptr_cap;
+  const bool vec2 = (N % 2 == 0) && (ldw % 2 == 0) && (ldt % 2 == 0) && ((reinterpret_cast<uintptr_t>(W) & 15u) == 0) &&
+                    ((reinterpret_cast<uintptr_t>(T) & 15u) == 0);
   const double one = 1.0, zero = 0.0;
   cudaStream_t st = h->stream;
   const unsigned ew = 148 * 16;
@@ -111,8 +132,9 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
     for (int64_t b0 = col.color_begin[k]; b0 < col.color_begin[k + 1]; b0 += cap) {
       const int64_t batch = std::min<int64_t>(cap, col.color_begin[k + 1] - b0);
       const int32_t *cells = col.cell_order + b0;
-      const int64_t rows = batch * nl;
-      feg_gather_kernel<<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows);
+      const int32_t rows = (int32_t)(batch * nl);
+      if (vec2) feg_gather_kernel<2><<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows);
+      else feg_gather_kernel<1><<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows);
       LAUNCH_CHECK(h);
       if (conv) {
         feg_convert_kernel<<<ew, 256, 0, st>>>(op.cell_mats_f32, cells, (int64_t)nl * nl, h->feg_A, op.cell_shared ? 1 : batch, op.cell_shared ? 1 : 0);
@@ -130,7 +152,8 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
         return RCHFSI_ECUDA;
       }
       h->launches++;
-      feg_scatter_kernel<<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows);
+      if (vec2) feg_scatter_kernel<2><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows);
+      else feg_scatter_kernel<1><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows);
       LAUNCH_CHECK(h);
     }
   return RCHFSI_OK;

@@ -246,6 +246,12 @@ rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n
       Gbuf = h->Gtmp;
     }
   }
+  {
+    // the filter's workspace first: the chunked Rayleigh-Ritz sizes its chunks from the memory that is left
+    const Plan pl = make_plan(h);
+    const bool chf = (method == RCHFSI_METHOD_CHFSI);
+    RCHFSI_TRY(ensure_filter_workspace(h, pl, degree, !chf && !g32 && (pl.store != RCHFSI_FP64 || pl.panel)));
+  }
   auto do_rr = [&]() -> rchfsi_status {
     if (chunked) return rayleigh_ritz_chunked(h, X, h->ritz_dev, Gbuf, g32 ? RCHFSI_FP32 : RCHFSI_FP64, h->res_dev);
     return rayleigh_ritz_impl(h, X, h->ritz_dev, (double *)Gbuf, h->res_dev);

@@ -223,7 +223,12 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   const int32_t N = h->N;
   cudaStream_t st = h->stream;
   if (!h->rrc1) {
-    int64_t cw = (int64_t)(6.0e9 / (16.0 * (double)m));
+    // two [m][cw] FP64 chunks: 6 GB, or up to a third of the free memory when there is more (wider chunks make the
+    // batched FE applies and the Gram GEMMs more efficient)
+    size_t free_b = 0, total_b = 0;
+    double budget = 6.0e9;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) budget = std::max(budget, 0.33 * ((double)free_b - 12.0e9));   // 12 GB kept for the low-precision operator copies and scratch still to come
+    int64_t cw = (int64_t)(budget / (16.0 * (double)m));
     cw = std::max<int64_t>(8, std::min<int64_t>(N, cw >= 48 ? cw / 48 * 48 : cw / 8 * 8));   // multiples of the FE column tile
     int64_t rp = (int64_t)(3.0e9 / (8.0 * (double)N));
     rp = std::max<int64_t>(256, std::min<int64_t>(m, rp));
@@ -235,6 +240,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   }
   const int32_t cw = h->rr_cw;
   const double one = 1.0, zero = 0.0;
+  PhaseTimer pt(h);
   if (h->opt.normalize_columns_before_rr) {
     RCHFSI_TRY(column_sumsq(h, RCHFSI_FP64, Y, m, N, h->colnorm));
     RCHFSI_TRY(scale_columns_inv_norm(h, Y, m, N, h->colnorm));
@@ -256,6 +262,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     }
     h->launches += 2;
   }
+  pt.lap("chunked: applies + Gram (lower)");
   CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
                                      CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,
                                      h->sy_lwork, h->sy_info));
@@ -268,6 +275,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
              (info > N ? " (Y^T B Y not positive definite)" : " (eigensolver did not converge)");
     return RCHFSI_EBREAKDOWN;
   }
+  pt.lap("chunked: dsygvd");
   const double *E = h->Ha;
   // X = Y E in place, one row panel at a time (row-major rows r0.. are the columns r0.. of the N x m view)
   for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
@@ -278,6 +286,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
                                          cudaMemcpyDeviceToDevice, st));
     h->launches++;
   }
+  pt.lap("chunked: X = Y E (row panels)");
   if (G_out || res_out) {
     // G = A X - B X Lambda recomputed from the rotated block, chunk by chunk (two more operator applies instead
     // of two more full-size temporaries)
@@ -297,6 +306,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
       RCHFSI_TRY(residual_window(h, h->rrc1, w, BX, ldb, h->ritz_dev + c0, Gc, N, g_prec, res_out ? res_out + c0 : nullptr, m, w));
     }
     if (res_out) RCHFSI_TRY(sqrt_inplace(h, res_out, N));
+    pt.lap("chunked: residual applies");
   }
   if (ritz_out && ritz_out != h->ritz_dev)
     RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz_out, h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));
