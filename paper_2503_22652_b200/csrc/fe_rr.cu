@@ -5,7 +5,7 @@
 // colour that touches a node writes, the later ones add (same first-touch flags as the tensor-core filter).
 // The filter's own FP64 mode keeps the hand-written kernel of kernels_simt.cu; this path only serves
 // rchfsi_rayleigh_ritz / rchfsi_solve, where the products are plain library GEMMs like the Gram and rotation
-// products next to them.  Measured at config 4: 158 -> see DESIGN.md section 8.
+// products next to them.  Config 4 (m = 912,673, N = 1200): 48 ms per apply against 158 ms.
 #include <algorithm>
 #include <cstdlib>
 #include "common.cuh"
