@@ -6,70 +6,89 @@
 namespace rchfsi {
 
 // ------------------------------------------------------------------------------------ dense
-// T[i][j] = sum_k A[i][k] * (dinv[k] * W[k][j]); 64x64 tile, 16x16 threads, 4x4 per thread.
-template <typename TC>
+// T[i][j] = sum_k A[i][k] * (dinv[k] * W[k][j]); BM x 64 tile, 16x16 threads, (BM/16) x 4 per thread, the next
+// K tile prefetched into registers while the current one is multiplied.
+// <64, 16> for large problems; <16, 64> when 64-row tiles would leave most SMs idle (config 1: 16 -> 63 CTAs, and
+// 16 instead of 63 exposed global-memory round trips along K).
+template <typename TC, int BM, int BK>
 __global__ void __launch_bounds__(256) dense_apply_kernel(const double *__restrict__ A, int64_t lda,
                                                           const double *__restrict__ dinv,
                                                           const TC *__restrict__ W, TC *__restrict__ T,
                                                           int64_t m, int32_t N, int64_t ldw, int64_t ldt) {
-  constexpr int BM = 64, BN = 64, BK = 16;
+  constexpr int BN = 64, RPT = BM / 16;
+  constexpr int NA = BM * BK / 256, NW = BK * BN / 256;
   __shared__ TC As[BK][BM + 4];
   __shared__ TC Ws[BK][BN + 4];
   const int tid = threadIdx.x;
   const int tx = tid & 15, ty = tid >> 4;
   const int64_t i0 = (int64_t)blockIdx.y * BM;
   const int j0 = blockIdx.x * BN;
-  TC acc[4][4];
+  TC acc[RPT][4];
 #pragma unroll
-  for (int r = 0; r < 4; ++r)
+  for (int r = 0; r < RPT; ++r)
 #pragma unroll
     for (int c = 0; c < 4; ++c) acc[r][c] = TC(0);
-  for (int64_t k0 = 0; k0 < m; k0 += BK) {
-    // A tile: 64 rows x 16 k, k fastest across threads
+  TC pa[NA], pw[NW];
+  auto fetch = [&](int64_t k0) {
+    // A tile: BM rows x BK k, k fastest across threads
 #pragma unroll
-    for (int l = 0; l < 4; ++l) {
-      int e = tid + l * 256;
-      int r = e >> 4, kk = e & 15;
-      int64_t i = i0 + r, k = k0 + kk;
-      As[kk][r] = (i < m && k < m) ? (TC)A[i * lda + k] : TC(0);
+    for (int l = 0; l < NA; ++l) {
+      const int e = tid + l * 256;
+      const int r = e / BK, kk = e % BK;
+      const int64_t i = i0 + r, k = k0 + kk;
+      pa[l] = (i < m && k < m) ? (TC)A[i * lda + k] : TC(0);
     }
-    // W tile: 16 k x 64 cols, scaled by dinv[k]
+    // W tile: BK k x 64 columns, scaled by dinv[k]
 #pragma unroll
-    for (int l = 0; l < 4; ++l) {
-      int e = tid + l * 256;
-      int kk = e >> 6, c = e & 63;
-      int64_t k = k0 + kk;
-      int j = j0 + c;
+    for (int l = 0; l < NW; ++l) {
+      const int e = tid + l * 256;
+      const int kk = e >> 6, c = e & 63;
+      const int64_t k = k0 + kk;
+      const int jc = j0 + c;
       TC v = TC(0);
-      if (k < m && j < N) {
-        v = W[k * ldw + j];
+      if (k < m && jc < N) {
+        v = W[k * ldw + jc];
         if (dinv) v = (TC)dinv[k] * v;
       }
-      Ws[kk][c] = v;
+      pw[l] = v;
+    }
+  };
+  fetch(0);
+  for (int64_t k0 = 0; k0 < m; k0 += BK) {
+#pragma unroll
+    for (int l = 0; l < NA; ++l) {
+      const int e = tid + l * 256;
+      As[e % BK][e / BK] = pa[l];
+    }
+#pragma unroll
+    for (int l = 0; l < NW; ++l) {
+      const int e = tid + l * 256;
+      Ws[e >> 6][e & 63] = pw[l];
     }
     __syncthreads();
+    if (k0 + BK < m) fetch(k0 + BK);
 #pragma unroll
     for (int kk = 0; kk < BK; ++kk) {
-      TC a[4], w[4];
+      TC a[RPT], w[4];
 #pragma unroll
-      for (int r = 0; r < 4; ++r) a[r] = As[kk][ty * 4 + r];
+      for (int r = 0; r < RPT; ++r) a[r] = As[kk][ty * RPT + r];
 #pragma unroll
       for (int c = 0; c < 4; ++c) w[c] = Ws[kk][tx * 4 + c];
 #pragma unroll
-      for (int r = 0; r < 4; ++r)
+      for (int r = 0; r < RPT; ++r)
 #pragma unroll
         for (int c = 0; c < 4; ++c) acc[r][c] += a[r] * w[c];
     }
     __syncthreads();
   }
 #pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    int64_t i = i0 + ty * 4 + r;
+  for (int r = 0; r < RPT; ++r) {
+    int64_t i = i0 + ty * RPT + r;
     if (i >= m) continue;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
-      int j = j0 + tx * 4 + c;
-      if (j < N) T[i * ldt + j] = acc[r][c];
+      int jj = j0 + tx * 4 + c;
+      if (jj < N) T[i * ldt + jj] = acc[r][c];
     }
   }
 }
@@ -162,8 +181,13 @@ rchfsi_status op_apply_simt(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   if (ldw == 0) ldw = N;
   if (ldt == 0) ldt = N;
   if (op.kind == RCHFSI_OP_DENSE) {
-    dim3 grid((unsigned)cdiv(N, 64), (unsigned)cdiv(m, 64));
-    dense_apply_kernel<TC><<<grid, 256, 0, st>>>(op.dense, op.lda, dinv_in, W, T, m, N, ldw, ldt);
+    if (cdiv(N, 64) * cdiv(m, 64) >= 148) {
+      dim3 grid((unsigned)cdiv(N, 64), (unsigned)cdiv(m, 64));
+      dense_apply_kernel<TC, 64, 16><<<grid, 256, 0, st>>>(op.dense, op.lda, dinv_in, W, T, m, N, ldw, ldt);
+    } else {
+      dim3 grid((unsigned)cdiv(N, 64), (unsigned)cdiv(m, 16));
+      dense_apply_kernel<TC, 16, 64><<<grid, 256, 0, st>>>(op.dense, op.lda, dinv_in, W, T, m, N, ldw, ldt);
+    }
     LAUNCH_CHECK(h);
   } else if (op.kind == RCHFSI_OP_CSR) {
     constexpr int V = (sizeof(TC) == 8) ? 2 : 4;
