@@ -119,6 +119,8 @@ rchfsi_status rchfsi_destroy(rchfsi_handle h) {
   for (void *p : h->owned) cudaFree(p);
   if (h->cublas) cublasDestroy(h->cublas);
   if (h->cusolver) cusolverDnDestroy(h->cusolver);
+  if (h->ev_x) cudaEventDestroy(h->ev_x);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->ev_step0) cudaEventDestroy(h->ev_step0);
   if (h->ev_step1) cudaEventDestroy(h->ev_step1);
   delete h;

@@ -90,8 +90,12 @@ struct rchfsi_ctx {
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
 
-  // host-buffer entry point scratch
+  // host-buffer entry point scratch; the H2D copy of X runs on copy_stream behind the recurrence (Alg. 3 reads X
+  // only in its last line) and the main stream waits for ev_x before the finish kernel
   double *hX = nullptr, *hG = nullptr, *hritz = nullptr;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_x = nullptr;
+  bool x_pending = false;
 
   // instrumentation
   cudaEvent_t ev_step0 = nullptr, ev_step1 = nullptr;

@@ -186,6 +186,10 @@ static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, con
   RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step1, st));
   h->last_steps = degree - 1;
 
+  if (h->x_pending) {   // rchfsi_filter_host: X is still arriving on the copy stream
+    h->x_pending = false;
+    RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(st, h->ev_x, 0));
+  }
   if (!chfsi)   // Y_p = D^-1 R_Y + X Lambda_Y
     RCHFSI_TRY(finish_block(h, pl.store, RY, h->dinv, h->lam_table + (size_t)degree * N, X, m, N, pm));
   else
@@ -211,11 +215,30 @@ rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host
   if (!h->hX) RCHFSI_TRY(dev_alloc(h, (void **)&h->hX, blk));
   if (!h->hritz) RCHFSI_TRY(dev_alloc(h, (void **)&h->hritz, sizeof(double) * h->N));
   if (G_host && !h->hG) RCHFSI_TRY(dev_alloc(h, (void **)&h->hG, blk));
-  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hX, X_host, blk, cudaMemcpyHostToDevice, st));
-  if (ritz_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * h->N, cudaMemcpyHostToDevice, st));
-  if (G_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hG, G_host, blk, cudaMemcpyHostToDevice, st));
-  RCHFSI_TRY(rchfsi_filter(h, method, h->hX, ritz_host ? h->hritz : nullptr, G_host ? h->hG : nullptr, degree,
-                           lam_min, lam_T, lam_max));
+  // Alg. 3 with the residual block given reads X only in its last line: its copy goes on a second
+  // stream and overlaps the p-1 recurrence steps; G and the Ritz values are needed first and go ahead of the kernels
+  h->x_pending = false;
+  const bool overlap_x = (method == RCHFSI_METHOD_RCHFSI) && G_host != nullptr;
+  if (overlap_x) {
+    if (!h->copy_stream) RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    if (!h->ev_x) RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_x, cudaEventDisableTiming));
+    if (G_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hG, G_host, blk, cudaMemcpyHostToDevice, st));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * h->N, cudaMemcpyHostToDevice, st));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hX, X_host, blk, cudaMemcpyHostToDevice, h->copy_stream));
+    RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_x, h->copy_stream));
+    h->x_pending = true;
+  } else {
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hX, X_host, blk, cudaMemcpyHostToDevice, st));
+    if (ritz_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * h->N, cudaMemcpyHostToDevice, st));
+    if (G_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hG, G_host, blk, cudaMemcpyHostToDevice, st));
+  }
+  rchfsi_status fst = rchfsi_filter(h, method, h->hX, ritz_host ? h->hritz : nullptr, G_host ? h->hG : nullptr, degree,
+                                    lam_min, lam_T, lam_max);
+  if (h->x_pending) {   // the filter returned before its last line (invalid arguments): do not leave the copy in flight
+    h->x_pending = false;
+    cudaStreamSynchronize(h->copy_stream);
+  }
+  RCHFSI_TRY(fst);
   RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(X_host, h->hX, blk, cudaMemcpyDeviceToHost, st));
   RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
   return RCHFSI_OK;
