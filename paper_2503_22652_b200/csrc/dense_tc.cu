@@ -218,6 +218,28 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       // then CTA z sums the BN / ks matrix rows it owns over the ranks in fixed order (deterministic)
       // and applies the update to them.
       float *part = reinterpret_cast<float *>(smem);
+      const int jl = threadIdx.x & 127;
+      const int jj = j0 + jl;
+      const bool jjok = jj < p.N && !(p.debug_mode & 4);
+      const S ly2 = (S)((G != nullptr && jjok) ? p.LY[jj] : 0.0);
+      const int cpr = BN / ks;                                  // matrix rows owned by this CTA
+      const int cbase = blockIdx.z * cpr + (threadIdx.x >> 7);  // this thread: every second owned row
+      const int nrow = cpr / 2;
+      // R_Y, R_X, G of 8 rows at a time; the first batch is requested before the partial tiles are exchanged and
+      // every later one while the current batch is summed, so only the first latency is exposed
+      S ry[8], rx[8], g[8], ryn[8], rxn[8], gn[8];
+      auto gload = [&](S (&a)[8], S (&b)[8], S (&c)[8], int u0) {
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          const int64_t i = i0 + cbase + 2 * (u0 + t);
+          const int64_t idx = i * p.N + jj;
+          const bool ok = jjok && (u0 + t) < nrow && i < p.m;
+          a[t] = ok ? __ldg(RY + idx) : S(0);
+          b[t] = ok ? RX[idx] : S(0);
+          c[t] = (ok && G) ? __ldg(G + idx) : S(0);
+        }
+      };
+      gload(ry, rx, g, 0);
 #pragma unroll 1
       for (int c0 = half * HALF_COLS; c0 < (half + 1) * HALF_COLS; c0 += 32) {
         uint32_t r[32];
@@ -227,53 +249,52 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
         for (int t = 0; t < 32; ++t) part[(c0 + t) * 128 + 32 * q + lane] = __uint_as_float(r[t]);
       }
       cluster_sync_all();
-      const int jl = threadIdx.x & 127;
-      const int jj = j0 + jl;
-      const bool jjok = jj < p.N;
-      const S ly2 = (S)((G != nullptr && jjok) ? p.LY[jj] : 0.0);
-      const int cpr = BN / ks;                                  // matrix rows owned by this CTA
-      const int cbase = blockIdx.z * cpr + (threadIdx.x >> 7);  // this thread: every second owned row
       const uint32_t part_s = smem_u32(part);
-      if (jjok && !(p.debug_mode & 4)) {
 #pragma unroll 1
-        for (int u0 = 0; u0 < cpr / 2; u0 += 8) {
-          S ry[8], rx[8], g[8];
-          float T[8];
+      for (int u0 = 0; u0 < nrow; u0 += 8) {
+        float T[8];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) T[t] = 0.f;
+        // all the partial sums of the batch are requested before the first is used (fixed rank order: deterministic)
+        for (int rr = 0; rr < ks; ++rr) {
+          const uint32_t base = dsmem_map(part_s, (p.debug_mode & 64) ? blockIdx.z : rr);   // bit 6: local reads only (timing probe)
+          float pv[8];
 #pragma unroll
           for (int t = 0; t < 8; ++t) {
             const int c = cbase + 2 * (u0 + t);
-            const int64_t i = i0 + c;
-            const int64_t idx = i * p.N + jj;
-            const bool ok = (u0 + t) < cpr / 2 && i < p.m;
-            ry[t] = ok ? __ldg(RY + idx) : S(0);
-            rx[t] = ok ? RX[idx] : S(0);
-            g[t] = (ok && G) ? __ldg(G + idx) : S(0);
-            float acc = 0.f;
-            if (ok)
-              for (int rr = 0; rr < ks; ++rr) acc += dsmem_ld_f32(dsmem_map(part_s, rr) + (uint32_t)(c * 128 + jl) * 4u);
-            T[t] = acc;
+            const bool ok = jjok && (u0 + t) < nrow && i0 + c < p.m;
+            pv[t] = ok ? dsmem_ld_f32(base + (uint32_t)(c * 128 + jl) * 4u) : 0.f;
           }
 #pragma unroll
-          for (int t = 0; t < 8; ++t) {
-            const int c = cbase + 2 * (u0 + t);
-            const int64_t i = i0 + c;
-            if ((u0 + t) < cpr / 2 && i < p.m) {
-              const int64_t idx = i * p.N + jj;
-              S Tt = (S)T[t];
-              if (p.dinv_out) Tt *= (S)p.dinv_out[i];
-              const S out = ka * Tt + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly2);
-              RX[idx] = out;
-              if (p.Wnext) {
-                if constexpr (KIND == 0) {
-                  uint32_t uu;
-                  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(uu) : "f"((float)out));
-                  reinterpret_cast<uint32_t *>(p.Wnext)[idx] = uu;
-                } else {
-                  reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
-                }
+          for (int t = 0; t < 8; ++t) T[t] += pv[t];
+        }
+        if (u0 + 8 < nrow) gload(ryn, rxn, gn, u0 + 8);
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          const int c = cbase + 2 * (u0 + t);
+          const int64_t i = i0 + c;
+          if (jjok && (u0 + t) < nrow && i < p.m) {
+            const int64_t idx = i * p.N + jj;
+            S Tt = (S)T[t];
+            if (p.dinv_out) Tt *= (S)p.dinv_out[i];
+            const S out = ka * Tt + kb_ * ry[t] + kc * rx[t] + ka * (g[t] * ly2);
+            RX[idx] = out;
+            if (p.Wnext) {
+              if constexpr (KIND == 0) {
+                uint32_t uu;
+                asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(uu) : "f"((float)out));
+                reinterpret_cast<uint32_t *>(p.Wnext)[idx] = uu;
+              } else {
+                reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
               }
             }
           }
+        }
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          ry[t] = ryn[t];
+          rx[t] = rxn[t];
+          g[t] = gn[t];
         }
       }
       cluster_sync_all();     // nobody leaves while its shared memory may still be read
@@ -414,15 +435,31 @@ bool dense_tc_supported(const rchfsi_ctx *h) {
   return false;
 }
 
-int dense_tc_pick_bn(int64_t m, int32_t N) {
-  if (const char *e = getenv("RCHFSI_DENSE_BN")) {   // tuning knob
+// Tile height BN (operator rows per CTA) and K splits.  Large problems: the widest tile that still gives a full
+// wave.  Mid-size problems (config 2: 2 x 32 tiles of 128 rows for 148 SMs): 128-row tiles with the K range split
+// over a 2-CTA cluster and the partial tiles summed through distributed shared memory -- 128 CTAs with an N = 128
+// MMA (96 cycles for twice the work of the 80-cycle N = 64 one) and 2/3 of the operand traffic of 64-row tiles;
+// measured 33.1 against 35.2 us per step.  Small problems: 64-row tiles.
+void dense_tc_pick(int64_t m, int32_t N, int nkb128, int *bn_out, int *ks_out) {
+  int bn = 0, ks = 1;
+  if (const char *e = getenv("RCHFSI_DENSE_BN")) {   // tuning knobs
     const int v = atoi(e);
-    if (v == 64 || v == 128 || v == 256) return v;
+    if (v == 64 || v == 128 || v == 256) bn = v;
   }
   const int64_t tj = cdiv(N, 128);
-  if (tj * cdiv(m, 256) >= 120) return 256;
-  if (tj * cdiv(m, 128) >= 120) return 128;
-  return 64;
+  if (bn == 0) {
+    const int64_t t128 = tj * cdiv(m, 128);
+    if (tj * cdiv(m, 256) >= 120) bn = 256;
+    else if (t128 >= 120) bn = 128;
+    else if (2 * t128 >= 100 && 2 * t128 <= 148 && nkb128 >= 8) { bn = 128; ks = 2; }
+    else bn = 64;
+  }
+  if (const char *e = getenv("RCHFSI_DENSE_KS")) {
+    const int v = atoi(e);
+    if (v == 1 || v == 2 || v == 4 || v == 8) ks = v;
+  }
+  *bn_out = bn;
+  *ks_out = ks;
 }
 
 rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
@@ -432,7 +469,10 @@ rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
   const LowpCopy *cp = get_dense_copy(h, bf16 ? RCHFSI_BF16 : RCHFSI_TF32, folded, &st);
   if (!cp) return st;
   const int eb = bf16 ? 2 : 4;
-  const int bn = dense_tc_pick_bn(h->m, h->N);
+  const int32_t nkb = (int32_t)cdiv(h->m, (bf16 ? 64 : 32) * 2);
+  int bn = 64, ks = 1;
+  dense_tc_pick(h->m, h->N, nkb, &bn, &ks);
+  while (ks > 1 && (nkb < 2 * ks || bn % (2 * ks) != 0)) ks /= 2;
   // W [m][N]: box = 128 B of block columns x (32 | 64) k rows
   const CUtensorMap *ptW = get_tmap_2d(h, s.W, eb, bf16, (uint64_t)h->m, (uint64_t)h->N, (uint64_t)h->N * eb,
                                        bf16 ? 64 : 32, bf16 ? 64 : 32, !bf16);
@@ -443,11 +483,6 @@ rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
     return RCHFSI_ECUDA;
   }
   const CUtensorMap tmW = *ptW, tmA = *ptA;
-  const int32_t nkb = (int32_t)cdiv(h->m, (bf16 ? 64 : 32) * 2);
-  int ks = 1;
-  if (const char *e = getenv("RCHFSI_DENSE_KS")) ks = atoi(e);     // tuning knob
-  if (ks != 1 && ks != 2 && ks != 4 && ks != 8) ks = 1;
-  while (ks > 1 && (nkb < 2 * ks || bn % (2 * ks) != 0)) ks /= 2;
   DenseTcParams p{s.k, s.RY, s.RX, s.G, s.LY, s.chfsi ? h->dinv : nullptr, s.Wnext, h->m, h->N,
                   nkb, ks, getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0};
   if (s.store_prec == RCHFSI_FP64)

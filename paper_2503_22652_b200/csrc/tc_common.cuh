@@ -61,9 +61,11 @@ __device__ __forceinline__ uint32_t dsmem_map(uint32_t local_saddr, uint32_t ran
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_saddr), "r"(rank));
   return r;
 }
+// not volatile: callers order these loads with cluster_sync_all() (which clobbers memory), and the compiler is free to
+// batch several of them ahead of their first use
 __device__ __forceinline__ float dsmem_ld_f32(uint32_t cluster_saddr) {
   float v;
-  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_saddr) : "memory");
+  asm("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_saddr));
   return v;
 }
 
