@@ -74,6 +74,7 @@ struct DenseTcParams {
   int32_t N;
   int32_t num_k_blocks;
   int32_t ksplit;       // K splits = cluster size along z (1, 2, 4 or 8)
+  int32_t mcast;        // 1: the two column tiles of a cluster (cluster x = 2) share the operator tile by TMA multicast
   int32_t debug_mode;   // 0 normal; 1 = no MMA (TMA throughput); 2 = no TMA (MMA throughput): timing probes only
 };
 
@@ -95,7 +96,8 @@ __device__ __forceinline__ double ld_s(const S *p) { return (double)*p; }
 // KIND 0: TF32 (FP32 bit patterns; W may be R_Y itself), KIND 1: BF16 operands.
 template <int KIND, int BN, typename S>
 __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant__ CUtensorMap tmW,
-                                                          const __grid_constant__ CUtensorMap tmA, DenseTcParams p) {
+                                                          const __grid_constant__ CUtensorMap tmA,
+                                                          const __grid_constant__ CUtensorMap tmAh, DenseTcParams p) {
   using Cfg = DenseCfg<BN>;
   constexpr int KR = KIND == 0 ? 32 : 64;       // K extent of one stage (128 B per operator row)
   extern __shared__ uint8_t smem_raw[];
@@ -114,12 +116,18 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
   const int kb_begin = (int)((int64_t)p.num_k_blocks * blockIdx.z / ks);
   const int nkb = (int)((int64_t)p.num_k_blocks * (blockIdx.z + 1) / ks) - kb_begin;
 
+  // multicast (p.mcast): cluster = (2 column tiles, 1, ks K-splits); the pair with the same z loads half of the
+  // operator tile each and delivers it to both, so a stage is free only when BOTH consumers have released it
+  const bool mc = p.mcast != 0;
+  const uint32_t cx = mc ? (blockIdx.x & 1u) : 0u;
+  const uint16_t pair_mask = mc ? (uint16_t)(3u << (2u * blockIdx.z)) : (uint16_t)0;
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmW);
     tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmAh);
     for (int s = 0; s < Cfg::STAGES; ++s) {
       mbar_init(full_bar + s, 1);
-      mbar_init(empty_bar + s, 1);
+      mbar_init(empty_bar + s, mc ? 2 : 1);
     }
     mbar_init(accum_bar, 1);
     fence_barrier_init();
@@ -127,6 +135,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
   if (warp == 2) tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
   tc_fence_before();
   __syncthreads();
+  if (mc) cluster_sync_all();     // every barrier of the cluster exists before the first remote arrival
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
@@ -153,7 +162,10 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
 #pragma unroll
               for (int a = 0; a < 2; ++a) tma_load_2d(ws + a * 8192, &tmW, full_bar + s, j0 + 64 * a, k0);
             }
-            tma_load_2d(as, &tmA, full_bar + s, k0, (int32_t)i0);
+            if (mc)
+              tma_load_2d_mc(as + cx * (BN / 2) * 128, &tmAh, full_bar + s, k0, (int32_t)(i0 + cx * (BN / 2)), pair_mask);
+            else
+              tma_load_2d(as, &tmA, full_bar + s, k0, (int32_t)i0);
           }
         }
       }
@@ -187,7 +199,8 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
               umma<KIND>(tmem_base, da, db, idesc, (kb > 0 || pn > 0 || q > 0) ? 1u : 0u);
             }
           }
-          umma_commit(empty_bar + s);
+          if (mc) umma_commit_mc(empty_bar + s, pair_mask);
+          else umma_commit(empty_bar + s);
         }
       }
       __syncwarp();
@@ -225,12 +238,13 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       const int cpr = BN / ks;                                  // matrix rows owned by this CTA
       const int cbase = blockIdx.z * cpr + (threadIdx.x >> 7);  // this thread: every second owned row
       const int nrow = cpr / 2;
-      // R_Y, R_X, G of 8 rows at a time; the first batch is requested before the partial tiles are exchanged and
+      // R_Y, R_X, G of RB rows at a time; the first batch is requested before the partial tiles are exchanged and
       // every later one while the current batch is summed, so only the first latency is exposed
-      S ry[8], rx[8], g[8], ryn[8], rxn[8], gn[8];
-      auto gload = [&](S (&a)[8], S (&b)[8], S (&c)[8], int u0) {
+      constexpr int RB = 16;
+      S ry[RB], rx[RB], g[RB];
+      auto gload = [&](S (&a)[RB], S (&b)[RB], S (&c)[RB], int u0) {
 #pragma unroll
-        for (int t = 0; t < 8; ++t) {
+        for (int t = 0; t < RB; ++t) {
           const int64_t i = i0 + cbase + 2 * (u0 + t);
           const int64_t idx = i * p.N + jj;
           const bool ok = jjok && (u0 + t) < nrow && i < p.m;
@@ -251,26 +265,26 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       cluster_sync_all();
       const uint32_t part_s = smem_u32(part);
 #pragma unroll 1
-      for (int u0 = 0; u0 < nrow; u0 += 8) {
-        float T[8];
+      for (int u0 = 0; u0 < nrow; u0 += RB) {
+        if (u0 > 0) gload(ry, rx, g, u0);
+        float T[RB];
 #pragma unroll
-        for (int t = 0; t < 8; ++t) T[t] = 0.f;
+        for (int t = 0; t < RB; ++t) T[t] = 0.f;
         // all the partial sums of the batch are requested before the first is used (fixed rank order: deterministic)
         for (int rr = 0; rr < ks; ++rr) {
-          const uint32_t base = dsmem_map(part_s, (p.debug_mode & 64) ? blockIdx.z : rr);   // bit 6: local reads only (timing probe)
-          float pv[8];
+          const uint32_t base = dsmem_map(part_s, ((p.debug_mode & 64) ? blockIdx.z : (uint32_t)rr) * (mc ? 2u : 1u) + cx);   // bit 6: local reads only (timing probe)
+          float pv[RB];
 #pragma unroll
-          for (int t = 0; t < 8; ++t) {
+          for (int t = 0; t < RB; ++t) {
             const int c = cbase + 2 * (u0 + t);
             const bool ok = jjok && (u0 + t) < nrow && i0 + c < p.m;
             pv[t] = ok ? dsmem_ld_f32(base + (uint32_t)(c * 128 + jl) * 4u) : 0.f;
           }
 #pragma unroll
-          for (int t = 0; t < 8; ++t) T[t] += pv[t];
+          for (int t = 0; t < RB; ++t) T[t] += pv[t];
         }
-        if (u0 + 8 < nrow) gload(ryn, rxn, gn, u0 + 8);
 #pragma unroll
-        for (int t = 0; t < 8; ++t) {
+        for (int t = 0; t < RB; ++t) {
           const int c = cbase + 2 * (u0 + t);
           const int64_t i = i0 + c;
           if (jjok && (u0 + t) < nrow && i < p.m) {
@@ -289,12 +303,6 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
               }
             }
           }
-        }
-#pragma unroll
-        for (int t = 0; t < 8; ++t) {
-          ry[t] = ryn[t];
-          rx[t] = rxn[t];
-          g[t] = gn[t];
         }
       }
       cluster_sync_all();     // nobody leaves while its shared memory may still be read
@@ -342,6 +350,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
   }
   tc_fence_before();
   __syncthreads();
+  if (mc && ks == 1) cluster_sync_all();   // the peer's last release still arrives on this CTA's barriers
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
@@ -394,7 +403,8 @@ const LowpCopy *get_dense_copy(rchfsi_ctx *h, int prec, bool folded, rchfsi_stat
 }
 
 template <int KIND, int BN, typename S>
-rchfsi_status launch_dense(rchfsi_ctx *h, const CUtensorMap &tmW, const CUtensorMap &tmA, const DenseTcParams &p) {
+rchfsi_status launch_dense(rchfsi_ctx *h, const CUtensorMap &tmW, const CUtensorMap &tmA, const CUtensorMap &tmAh,
+                           const DenseTcParams &p) {
   using Cfg = DenseCfg<BN>;
   auto kern = dense_tc_kernel<KIND, BN, S>;
   static bool attr_set = false;
@@ -409,21 +419,22 @@ rchfsi_status launch_dense(rchfsi_ctx *h, const CUtensorMap &tmW, const CUtensor
   cfg.stream = h->stream;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;     // the K splits of a tile form one cluster
-  attr[0].val.clusterDim.x = 1;
+  attr[0].val.clusterDim.x = p.mcast ? 2 : 1;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = (unsigned)p.ksplit;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  RCHFSI_CUDA_CHECK(h, cudaLaunchKernelEx(&cfg, kern, tmW, tmA, p));
+  RCHFSI_CUDA_CHECK(h, cudaLaunchKernelEx(&cfg, kern, tmW, tmA, tmAh, p));
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }
 
 template <int KIND, typename S>
-rchfsi_status launch_dense_bn(rchfsi_ctx *h, int bn, const CUtensorMap &tmW, const CUtensorMap &tmA, const DenseTcParams &p) {
-  if (bn == 256) return launch_dense<KIND, 256, S>(h, tmW, tmA, p);
-  if (bn == 128) return launch_dense<KIND, 128, S>(h, tmW, tmA, p);
-  return launch_dense<KIND, 64, S>(h, tmW, tmA, p);
+rchfsi_status launch_dense_bn(rchfsi_ctx *h, int bn, const CUtensorMap &tmW, const CUtensorMap &tmA, const CUtensorMap &tmAh,
+                              const DenseTcParams &p) {
+  if (bn == 256) return launch_dense<KIND, 256, S>(h, tmW, tmA, tmAh, p);
+  if (bn == 128) return launch_dense<KIND, 128, S>(h, tmW, tmA, tmAh, p);
+  return launch_dense<KIND, 64, S>(h, tmW, tmA, tmAh, p);
 }
 
 }  // namespace
@@ -478,16 +489,23 @@ rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
                                        bf16 ? 64 : 32, bf16 ? 64 : 32, !bf16);
   const CUtensorMap *ptA = get_tmap_2d(h, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb,
                                        bf16 ? 64 : 32, (uint32_t)bn);
-  if (!ptW || !ptA) {
+  // half-height operator tile for the multicast pair (each CTA fetches one half for both)
+  const CUtensorMap *ptAh = get_tmap_2d(h, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb,
+                                        bf16 ? 64 : 32, (uint32_t)bn / 2);
+  if (!ptW || !ptA || !ptAh) {
     h->err = "cuTensorMapEncodeTiled failed";
     return RCHFSI_ECUDA;
   }
-  const CUtensorMap tmW = *ptW, tmA = *ptA;
+  const CUtensorMap tmW = *ptW, tmA = *ptA, tmAh = *ptAh;
+  int mcast = (cdiv(h->N, 128) % 2 == 0 && 2 * ks <= 8) ? 1 : 0;
+  if (const char *e = getenv("RCHFSI_DENSE_MC")) mcast = mcast && atoi(e) != 0;   // tuning knob
+  const int dbg = getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0;
+  if (dbg & 3) mcast = 0;                                                          // the timing probes assume one consumer per stage
   DenseTcParams p{s.k, s.RY, s.RX, s.G, s.LY, s.chfsi ? h->dinv : nullptr, s.Wnext, h->m, h->N,
-                  nkb, ks, getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0};
+                  nkb, ks, mcast, dbg};
   if (s.store_prec == RCHFSI_FP64)
-    return bf16 ? launch_dense_bn<1, double>(h, bn, tmW, tmA, p) : launch_dense_bn<0, double>(h, bn, tmW, tmA, p);
-  return bf16 ? launch_dense_bn<1, float>(h, bn, tmW, tmA, p) : launch_dense_bn<0, float>(h, bn, tmW, tmA, p);
+    return bf16 ? launch_dense_bn<1, double>(h, bn, tmW, tmA, tmAh, p) : launch_dense_bn<0, double>(h, bn, tmW, tmA, tmAh, p);
+  return bf16 ? launch_dense_bn<1, float>(h, bn, tmW, tmA, tmAh, p) : launch_dense_bn<0, float>(h, bn, tmW, tmA, tmAh, p);
 }
 
 }  // namespace rchfsi

@@ -416,6 +416,35 @@ def test_dense_split_k_cluster_fixup_matches_unsplit(monkeypatch, bn, ks):
     assert rel_fro(outs[1], outs[0]) < 2.0 ** -11
 
 
+@pytest.mark.parametrize("apply_prec", ["tf32", "bf16"])
+@pytest.mark.parametrize("bn,ks", [(64, 1), (128, 2), (128, 1)])
+def test_dense_operator_tile_multicast_is_bitwise_the_unicast_result(monkeypatch, apply_prec, bn, ks):
+    """With an even number of column tiles the two column-tile CTAs of a cluster fetch half of the operator tile
+    each and deliver it to both by TMA multicast (RCHFSI_DENSE_MC=0 switches it off).  Only the data path
+    changes, not the arithmetic: the filtered blocks must be bitwise equal, with and without K splits, including
+    a ragged last row tile (m = 1000) and a ragged second column tile (N = 200)."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(1000, seed=78)
+    N, p = 200, 4
+    monkeypatch.setenv("RCHFSI_DENSE_BN", str(bn))
+    monkeypatch.setenv("RCHFSI_DENSE_KS", str(ks))
+    outs = []
+    for mc in ("1", "0"):
+        monkeypatch.setenv("RCHFSI_DENSE_MC", mc)
+        solver, (A, B, Dinv), X, ritz, G = _setup(prob, N, 14, apply_prec=apply_prec)
+        ev, top = _bounds(prob, A, B)
+        b = (ev[0] - 1e-3, ev[N], top * 1.01)
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+        outs.append(Xd.cpu().numpy())
+        solver.close()
+    assert np.array_equal(outs[0], outs[1])
+    # and it is the oracle's block up to operand rounding (same bound as the per-step test)
+    Yo = orc.filter_rchfsi(A.apply, Dinv.apply, X, ritz, G, p, *b)
+    assert rel_fro(outs[0], Yo) < (6e-3 if apply_prec == "tf32" else 3e-2)
+
+
 @pytest.mark.parametrize("kind", ["fe", "csr"])
 def test_fp32_residual_block_input_is_used_in_place(kind):
     """g_input_f32 (config-5 memory plan: an FP64 G does not fit): the filter with G given in FP32 equals the
