@@ -158,6 +158,7 @@ size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B
   if (A->kind == RCHFSI_OP_DENSE && o.apply_prec != RCHFSI_FP64) total += (size_t)A->m * A->m * 4;
   if (A->kind == RCHFSI_OP_FE && o.apply_prec != RCHFSI_FP64)
     total += (size_t)A->n_cells * 352 * 352 * (o.apply_prec == RCHFSI_BF16 ? 2 : 4);
+  if (A->kind == RCHFSI_OP_FE) total += (size_t)1600 << 20;   // gather / product / FP64 cell-batch scratch of the Rayleigh-Ritz applies
   return total;
 }
 
