@@ -46,9 +46,39 @@ __device__ __forceinline__ void st4(float *p, const double (&o)[4]) {
   *reinterpret_cast<float4 *>(p) = make_float4((float)o[0], (float)o[1], (float)o[2], (float)o[3]);
 }
 
-// S = storage type of R_X, R_Y, G (double or float).  Each CTA owns ROWS consecutive rows so
-// that the +-1 (and, for narrow grids, +-n) neighbour rows it re-reads are L1 hits.
-template <typename S, int ROWS>
+// Raw 4-element vectors of the storage type (two 16-byte words for FP64, one for FP32) so the loads of
+// R_X and G can be issued before the gather loop and converted after it.
+template <typename S> struct Vec4;
+template <> struct Vec4<double> { double2 lo, hi; };
+template <> struct Vec4<float> { float4 v; };
+__device__ __forceinline__ Vec4<double> ld4_stream(const double *p) {
+  Vec4<double> r;
+  r.lo = __ldcs(reinterpret_cast<const double2 *>(p));
+  r.hi = __ldcs(reinterpret_cast<const double2 *>(p + 2));
+  return r;
+}
+__device__ __forceinline__ Vec4<float> ld4_stream(const float *p) {
+  Vec4<float> r;
+  r.v = __ldcs(reinterpret_cast<const float4 *>(p));
+  return r;
+}
+__device__ __forceinline__ void unpack(const Vec4<double> &x, double (&o)[4]) { o[0] = x.lo.x; o[1] = x.lo.y; o[2] = x.hi.x; o[3] = x.hi.y; }
+__device__ __forceinline__ void unpack(const Vec4<float> &x, double (&o)[4]) { o[0] = x.v.x; o[1] = x.v.y; o[2] = x.v.z; o[3] = x.v.w; }
+__device__ __forceinline__ void st4_stream(double *p, const double (&o)[4]) {
+  __stcs(reinterpret_cast<double2 *>(p), make_double2(o[0], o[1]));
+  __stcs(reinterpret_cast<double2 *>(p + 2), make_double2(o[2], o[3]));
+}
+__device__ __forceinline__ void st4_stream(float *p, const double (&o)[4]) {
+  __stcs(reinterpret_cast<float4 *>(p), make_float4((float)o[0], (float)o[1], (float)o[2], (float)o[3]));
+}
+
+// S = storage type of R_X, R_Y, G (double or float).  Each CTA owns ROWS consecutive rows (and, with
+// gridDim.y > 1, one strip of the 4-column vectors) so that the +-1 neighbour rows it re-reads are L1 hits.
+// A thread owns one 4-column vector of one row.  Its streaming operands (R_X, G: touched once per
+// step, evict-first) are requested BEFORE the gather loop so their DRAM latency runs under it, and the
+// gather is unrolled UNR nonzeros deep: UNR column indices / values first, then UNR independent operand
+// loads, then the FMAs -- (UNR + 2) 16/32-byte requests in flight per thread instead of one.
+template <typename S, int ROWS, int UNR>
 __global__ void __launch_bounds__(256) csr_fused_kernel(const int64_t *__restrict__ rowptr,
                                                         const int32_t *__restrict__ colind,
                                                         const float *__restrict__ valsf,
@@ -56,36 +86,54 @@ __global__ void __launch_bounds__(256) csr_fused_kernel(const int64_t *__restric
                                                         const S *__restrict__ RY, S *__restrict__ RX,
                                                         const S *__restrict__ G, const double *__restrict__ LY,
                                                         StepCoef k, int64_t m, int32_t N) {
-  const int nvec = N >> 2;
+  const int nvec_all = N >> 2;
+  const int vper = (nvec_all + (int)gridDim.y - 1) / (int)gridDim.y;
+  const int v0 = (int)blockIdx.y * vper;
+  const int nvec = min(vper, nvec_all - v0);
+  if (nvec <= 0) return;
   const int64_t r0 = (int64_t)blockIdx.x * ROWS;
   const int items = ROWS * nvec;
   for (int it = threadIdx.x; it < items; it += blockDim.x) {
     const int rl = it / nvec;
-    const int v = it - rl * nvec;
+    const int v = v0 + (it - rl * nvec);
     const int64_t row = r0 + rl;
     if (row >= m) break;
+    const int64_t idx = row * N + 4 * v;
+    const Vec4<S> rxv = ld4_stream(RX + idx);
+    Vec4<S> gv;
+    if (G) gv = ld4_stream(G + idx);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     const int64_t t1 = rowptr[row + 1];
-    for (int64_t t = rowptr[row]; t < t1; ++t) {
-      const int32_t col = colind[t];
-      const float a = valsf[t];
-      const float4 w = ld4_as_float(RY + (int64_t)col * N + 4 * v);
-      acc.x = fmaf(a, w.x, acc.x);
-      acc.y = fmaf(a, w.y, acc.y);
-      acc.z = fmaf(a, w.z, acc.z);
-      acc.w = fmaf(a, w.w, acc.w);
+    for (int64_t t = rowptr[row]; t < t1; t += UNR) {
+      int32_t col[UNR];
+      float a[UNR];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) {
+        const bool ok = t + u < t1;
+        col[u] = ok ? colind[t + u] : (int32_t)row;
+        a[u] = ok ? valsf[t + u] : 0.f;
+      }
+      float4 w[UNR];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) w[u] = ld4_as_float(RY + (int64_t)col[u] * N + 4 * v);
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) {
+        acc.x = fmaf(a[u], w[u].x, acc.x);
+        acc.y = fmaf(a[u], w[u].y, acc.y);
+        acc.z = fmaf(a[u], w[u].z, acc.z);
+        acc.w = fmaf(a[u], w[u].w, acc.w);
+      }
     }
-    const int64_t idx = row * N + 4 * v;
     double ry[4], rx[4], out[4];
     ld4_as_double(RY + idx, ry);
-    ld4_as_double(RX + idx, rx);
+    unpack(rxv, rx);
     const double ds = dinv_out ? dinv_out[row] : 1.0;
     const double T[4] = {(double)acc.x, (double)acc.y, (double)acc.z, (double)acc.w};
 #pragma unroll
     for (int q = 0; q < 4; ++q) out[q] = k.a * (ds * T[q]) + k.b * ry[q] + k.cp * rx[q];
     if (G) {
       double g[4];
-      ld4_as_double(G + idx, g);
+      unpack(gv, g);
       const double2 l0 = *reinterpret_cast<const double2 *>(LY + 4 * v);
       const double2 l1 = *reinterpret_cast<const double2 *>(LY + 4 * v + 2);
       out[0] += k.a * (g[0] * l0.x);
@@ -93,7 +141,7 @@ __global__ void __launch_bounds__(256) csr_fused_kernel(const int64_t *__restric
       out[2] += k.a * (g[2] * l1.x);
       out[3] += k.a * (g[3] * l1.y);
     }
-    st4(RX + idx, out);
+    st4_stream(RX + idx, out);
   }
 }
 
@@ -126,25 +174,35 @@ rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s) {
     cp = &h->lowp.back();
   }
   const double *dinv_out = s.chfsi ? h->dinv : nullptr;
-  int rows = 32;
-  if (const char *e = getenv("RCHFSI_CSR_ROWS")) rows = atoi(e);   // tuning knob
-  auto launch = [&](auto rows_tag) {
+  int rows = 64, unr = 1, csplit = 1;
+  if (const char *e = getenv("RCHFSI_CSR_ROWS")) rows = atoi(e);       // tuning knobs
+  if (const char *e = getenv("RCHFSI_CSR_UNR")) unr = atoi(e);
+  if (const char *e = getenv("RCHFSI_CSR_CSPLIT")) csplit = std::max(1, atoi(e));
+  auto launch = [&](auto rows_tag, auto unr_tag) {
     constexpr int ROWS = decltype(rows_tag)::value;
-    const unsigned grid = (unsigned)cdiv(h->m, ROWS);
+    constexpr int UNR = decltype(unr_tag)::value;
+    const dim3 grid((unsigned)cdiv(h->m, ROWS), (unsigned)csplit);
     if (s.store_prec == RCHFSI_FP64)
-      csr_fused_kernel<double, ROWS><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
-                                                                   (const double *)s.RY, (double *)s.RX,
-                                                                   (const double *)s.G, s.LY, s.k, h->m, h->N);
+      csr_fused_kernel<double, ROWS, UNR><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
+                                                                        (const double *)s.RY, (double *)s.RX,
+                                                                        (const double *)s.G, s.LY, s.k, h->m, h->N);
     else
-      csr_fused_kernel<float, ROWS><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
-                                                                  (const float *)s.RY, (float *)s.RX,
-                                                                  (const float *)s.G, s.LY, s.k, h->m, h->N);
+      csr_fused_kernel<float, ROWS, UNR><<<grid, 256, 0, h->stream>>>(op.rowptr, op.colind, (const float *)cp->data, dinv_out,
+                                                                       (const float *)s.RY, (float *)s.RX,
+                                                                       (const float *)s.G, s.LY, s.k, h->m, h->N);
   };
-  if (rows == 8) launch(std::integral_constant<int, 8>{});
-  else if (rows == 16) launch(std::integral_constant<int, 16>{});
-  else if (rows == 64) launch(std::integral_constant<int, 64>{});
-  else if (rows == 128) launch(std::integral_constant<int, 128>{});
-  else launch(std::integral_constant<int, 32>{});
+  auto by_unr = [&](auto rows_tag) {
+    if (unr == 1) launch(rows_tag, std::integral_constant<int, 1>{});
+    else if (unr == 2) launch(rows_tag, std::integral_constant<int, 2>{});
+    else if (unr == 8) launch(rows_tag, std::integral_constant<int, 8>{});
+    else launch(rows_tag, std::integral_constant<int, 4>{});
+  };
+  if (rows == 8) by_unr(std::integral_constant<int, 8>{});
+  else if (rows == 16) by_unr(std::integral_constant<int, 16>{});
+  else if (rows == 64) by_unr(std::integral_constant<int, 64>{});
+  else if (rows == 128) by_unr(std::integral_constant<int, 128>{});
+  else if (rows == 256) by_unr(std::integral_constant<int, 256>{});
+  else by_unr(std::integral_constant<int, 32>{});
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }

@@ -1,6 +1,7 @@
 // rchfsi_filter / rchfsi_filter_host / rchfsi_solve: host control flow of Algorithm 2
 // (PAPER.md:78-86), Algorithm 3 and Algorithm 1.
 #include <cmath>
+#include <cstdlib>
 #include "common.cuh"
 
 using namespace rchfsi;
@@ -14,6 +15,7 @@ struct Plan {
   bool shadow;   // operand block is a separate buffer
   int fused;     // 0 unfused SIMT, 1 CSR fused, 2 dense tensor-core, 3 FE tensor-core
   bool panel;    // library-owned blocks in panel layout [ceil(N/128)][m][128] (FE tensor-core path)
+  bool shadow_inplace;   // one shadow buffer, overwritten in place by the fused FE step (see make_plan)
 };
 
 Plan make_plan(const rchfsi_ctx *h) {
@@ -36,6 +38,13 @@ Plan make_plan(const rchfsi_ctx *h) {
   p.tprec = (ap == RCHFSI_FP64) ? RCHFSI_FP64 : RCHFSI_FP32;
   p.shadow = (p.operand != p.store);
   p.panel = (p.fused == 3);
+  // FE step: the (cell, column tile) CTA that is the LAST toucher of a node writes the shadow row of the finished
+  // R_X value.  Every CTA that gathers that row for the same column tile belongs to a cell containing the node,
+  // i.e. to an earlier colour launch (complete, stream order) or to the writing CTA itself, whose gather ends
+  // before its epilogue starts: the new shadow may overwrite the old one, one buffer instead of two
+  // (14.8 GB instead of 29.6 GB of BF16 shadows at config 5).  The dense step cannot: its row tiles read all rows.
+  // RCHFSI_FE_SHADOW_PAIR=1 keeps the two-buffer scheme (the tests compare the two bit for bit).
+  p.shadow_inplace = p.shadow && p.fused == 3 && !getenv("RCHFSI_FE_SHADOW_PAIR");
   return p;
 }
 
@@ -44,8 +53,9 @@ rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t deg
   if (!h->RX) RCHFSI_TRY(dev_alloc(h, &h->RX, el * prec_bytes(pl.store)));
   if (!h->RY) RCHFSI_TRY(dev_alloc(h, &h->RY, el * prec_bytes(pl.store)));
   if (pl.shadow) {
-    if (!h->Wa) RCHFSI_TRY(dev_alloc(h, &h->Wa, el * 4));
-    if (!h->Wb) RCHFSI_TRY(dev_alloc(h, &h->Wb, el * 4));
+    const size_t wb = el * (pl.operand == RCHFSI_BF16 ? 2 : 4);
+    if (!h->Wa) RCHFSI_TRY(dev_alloc(h, &h->Wa, wb));
+    if (!pl.shadow_inplace && !h->Wb) RCHFSI_TRY(dev_alloc(h, &h->Wb, wb));
   }
   if (pl.fused == 0 && !h->T) RCHFSI_TRY(dev_alloc(h, &h->T, el * prec_bytes(pl.tprec)));
   if (need_gs && !h->Gs) RCHFSI_TRY(dev_alloc(h, &h->Gs, el * prec_bytes(pl.store)));
@@ -122,7 +132,7 @@ static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, con
   double sigma = sigma1;
 
   void *RX = h->RX, *RY = h->RY;
-  void *Wcur = pl.shadow ? h->Wa : nullptr, *Wnext = pl.shadow ? h->Wb : nullptr;
+  void *Wcur = pl.shadow ? h->Wa : nullptr, *Wnext = pl.shadow ? (pl.shadow_inplace ? h->Wa : h->Wb) : nullptr;
   const void *Gst = nullptr;
   uint64_t apply_index = 0;
 

@@ -335,6 +335,35 @@ def test_fe_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_pre
         solver.close()
 
 
+@pytest.mark.parametrize("apply_prec,store", [("bf16", "fp32"), ("bf16", "fp64"), ("tf32", "fp64")])
+def test_fe_shadow_block_updated_in_place_equals_the_two_buffer_scheme(monkeypatch, apply_prec, store):
+    """The FE step keeps ONE operand-precision shadow of R_Y and lets the last toucher of a node overwrite
+    its row in place (filter.cu make_plan: every reader of that row belongs to an earlier colour launch or is
+    the writer itself).  Bit-for-bit the same filtered block as the two-buffer scheme, over several steps,
+    three column tiles (ragged last) and a 3^3-cell mesh where interior nodes have 8 touchers."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.fe_problem(3, q=3, seed=41)
+    lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    N, p = 264, 7
+    out = {}
+    for pair in ("1", None):
+        if pair:
+            monkeypatch.setenv("RCHFSI_FE_SHADOW_PAIR", pair)
+        else:
+            monkeypatch.delenv("RCHFSI_FE_SHADOW_PAIR", raising=False)
+        solver, _, X, ritz, G = _setup(prob, N, 29, apply_prec=apply_prec, store_prec=store)
+        b = (ritz[0] - 1.0, ritz[-1] + 1.0, lam_max)
+        for method in (P.METHOD_RCHFSI, P.METHOD_CHFSI):
+            Xd = torch.as_tensor(X).cuda()
+            solver.filter(method, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+            out[(pair, method)] = Xd.cpu().numpy()
+        solver.close()
+    for method in (P.METHOD_RCHFSI, P.METHOD_CHFSI):
+        assert np.isfinite(out[(None, method)]).all()
+        assert np.array_equal(out[("1", method)], out[(None, method)])
+
+
 @pytest.mark.parametrize("kind", ["dense", "fe"])
 @pytest.mark.parametrize("apply_prec", ["tf32", "bf16"])
 def test_tensor_core_paths_edge_shapes(kind, apply_prec):
