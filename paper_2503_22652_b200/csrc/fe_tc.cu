@@ -225,8 +225,8 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
         for (int hsel = 0; hsel < 2; ++hsel) {
           const int a = c * R + sub * RW + t_lane + RSTEP * hsel;
           const uint32_t w = (a < p.n_loc && colok) ? rw_s[a] : 0u;
-          const bool valid = (a < p.n_loc) && colok;
-          const bool first = (w >> 30) & 1u;
+          const bool valid = (a < p.n_loc) && colok && !(p.debug_mode & 2048);     // bit 11: no epilogue loads (timing probe)
+          const bool first = ((w >> 30) & 1u) && !(p.debug_mode & 4096);           // bit 12: no R_Y / G loads (timing probe)
           const uint64_t off = (uint64_t)(w & 0x3FFFFFFFu) * (128 * sizeof(S)) + col_bytes;
           uint8_t *d = slot + dst_lane + hsel * (RSTEP * SEG);
           cp_async16(d, srcRX + off, valid ? 16u : 0u);
@@ -273,8 +273,8 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
               out = ka * T + kb_ * rys[t * 32 + lane] + kc * rxs[t * 32 + lane] + ka * (gs[t * 32 + lane] * ly);
             else
               out = rxs[t * 32 + lane] + ka * T;
-            RX[idx] = out;
-            if (p.Wnext && (flt & 2u)) {
+            if (!(p.debug_mode & 1024)) RX[idx] = out;                             // bit 10: no stores (timing probe)
+            if (p.Wnext && (flt & 2u) && !(p.debug_mode & 1024)) {
               if constexpr (KIND == 0) {
                 uint32_t u;
                 asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"((float)out));
