@@ -38,14 +38,6 @@ __device__ __forceinline__ void ld4_as_double(const float *p, double (&o)[4]) {
   const float4 a = *reinterpret_cast<const float4 *>(p);
   o[0] = a.x; o[1] = a.y; o[2] = a.z; o[3] = a.w;
 }
-__device__ __forceinline__ void st4(double *p, const double (&o)[4]) {
-  *reinterpret_cast<double2 *>(p) = make_double2(o[0], o[1]);
-  *reinterpret_cast<double2 *>(p + 2) = make_double2(o[2], o[3]);
-}
-__device__ __forceinline__ void st4(float *p, const double (&o)[4]) {
-  *reinterpret_cast<float4 *>(p) = make_float4((float)o[0], (float)o[1], (float)o[2], (float)o[3]);
-}
-
 // Raw 4-element vectors of the storage type (two 16-byte words for FP64, one for FP32) so the loads of
 // R_X and G can be issued before the gather loop and converted after it.
 template <typename S> struct Vec4;

@@ -77,7 +77,9 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   constexpr int R = 4 * RW;                            // rows per chunk over the 4 row-quarters
   constexpr int SEG = 32 * (int)sizeof(S);             // bytes of one row segment (32 columns)
   extern __shared__ uint8_t smem_raw[];
-  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  // 1 KB alignment as an OFFSET from the shared array: a pointer rebuilt from an integer loses its address
+  // space and every later access compiles to a generic LD/ST with 64-bit address math instead of LDS/STS
+  uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   const int stage_bytes = FE_W_BYTES + p.np * 128;
   const int main_bytes = max(FE_STAGES * stage_bytes, FE_WORK_WARPS * FE_DEPTH * FE_SLOT_BYTES);
   uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem + main_bytes);
@@ -95,8 +97,8 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   const int npanels = (p.debug_mode & 512) ? 0 : (p.ksteps * KSTEP + KR - 1) / KR;   // bit 9: fixed-cost probe
   const uint32_t tmem_cols = (p.np <= 32) ? 32u : (p.np <= 64 ? 64u : (p.np <= 128 ? 128u : (p.np <= 256 ? 256u : 512u)));
 
-  for (int t = threadIdx.x; t < p.n_loc; t += blockDim.x)
-    rw_s[t] = (uint32_t)(blockIdx.x * p.m + p.conn[cell * p.n_loc + t]) | ((uint32_t)p.flags[cell * p.n_loc + t] << 30);
+  for (int t = threadIdx.x; t < ((p.n_loc + 31) & ~31); t += blockDim.x)      // zero padded to whole chunks
+    rw_s[t] = t < p.n_loc ? ((uint32_t)(blockIdx.x * p.m + p.conn[cell * p.n_loc + t]) | ((uint32_t)p.flags[cell * p.n_loc + t] << 30)) : 0u;
   if (warp == FE_WORK_WARPS && lane == 0) {
     tma_prefetch_desc(&tmA);
     for (int s = 0; s < FE_STAGES; ++s) {
@@ -195,96 +197,139 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     }
 
     // ===== epilogue =====
+    // The epilogue is instruction-issue bound (16 warps, one element per lane and row: with every global
+    // access disabled it still takes ~14 us of the 26 us tile), so everything lane- or tile-constant is
+    // hoisted: per-lane base pointers (one IMAD.WIDE per address), the node words of a chunk as 128-bit
+    // shared loads, chunks that lie fully inside n_loc without per-row range checks, uniform branches
+    // around the rarely used pieces (dinv on the output rows, shadow store, row-major G).
     const int q4 = warp & 3;
     const int sub = warp >> 2;
     const int jl = 32 * q4 + lane;
     const int j = j0 + jl;
     const bool jok = j < p.N;
-    S *__restrict__ RX = reinterpret_cast<S *>(p.RX);
-    const uint8_t *srcRX = reinterpret_cast<const uint8_t *>(p.RX);
-    const uint8_t *srcRY = reinterpret_cast<const uint8_t *>(p.RY);
-    const uint8_t *srcG = reinterpret_cast<const uint8_t *>(p.G);
+    const bool do_store = jok && !(p.debug_mode & 1024);           // bit 10: no stores (timing probe)
+    const bool has_shadow = p.Wnext != nullptr;
+    const uint32_t tile_m = (uint32_t)(blockIdx.x * p.m);
+    constexpr uint32_t ROWB = 128 * sizeof(S);          // bytes of one row of a panel
+    constexpr uint32_t WB = KIND == 0 ? 4 : 2;          // shadow element bytes
+    const uint64_t rx_lane = (uint64_t)__cvta_generic_to_global(p.RX) + (uint64_t)jl * sizeof(S);
+    const uint64_t wn_lane = has_shadow ? (uint64_t)__cvta_generic_to_global(p.Wnext) + (uint64_t)jl * WB : 0;
     // the update runs in the storage precision (FP32 storage: FP32 arithmetic)
     const S ly = (S)((has_g && jok) ? p.LY[j] : 0.0);
     const S ka = (S)p.k.a, kb_ = (S)p.k.b, kc = (S)p.k.cp;
     const int nchunks = (p.n_loc + R - 1) / R;
     uint8_t *ring = smem + warp * (FE_DEPTH * FE_SLOT_BYTES);
     // one slot = [array 0..2][RW rows][SEG bytes] = 192 16-byte pieces, 6 per lane: a lane copies the same
-    // 16-byte column piece of two rows (h = 0, 1) for the three arrays; everything lane-constant is hoisted
+    // 16-byte column piece of two rows (h = 0, 1) for the three arrays
     constexpr int PPR = SEG / 16;                       // pieces per row segment: 8 (FP32) / 16 (FP64)
     constexpr int RSTEP = 32 / PPR;                     // rows covered by the 32 lanes: 4 / 2
     const int t_lane = lane / PPR;
     const int pc = lane % PPR;
-    const bool colok = j0 + 32 * q4 + pc * (16 / (int)sizeof(S)) < p.N;
+    const bool colok = j0 + 32 * q4 + pc * (16 / (int)sizeof(S)) < p.N && !(p.debug_mode & 2048);   // bit 11: no epilogue loads (probe)
     const uint32_t col_bytes = (uint32_t)(32 * q4 * (int)sizeof(S) + pc * 16);
-    const uint32_t dst_lane = (uint32_t)(t_lane * SEG + pc * 16);
+    const uint64_t srcRX = (uint64_t)__cvta_generic_to_global(p.RX) + col_bytes;
+    const uint64_t srcRY = (uint64_t)__cvta_generic_to_global(p.RY) + col_bytes;
+    // G: panel layout like R_X / R_Y, or the caller's own row-major block [m][N] (g_rowmajor)
+    const bool g_rm = p.g_rowmajor != 0;
+    const uint32_t g_rowb = g_rm ? (uint32_t)p.N * (uint32_t)sizeof(S) : ROWB;
+    const uint32_t g_sub = g_rm ? tile_m : 0u;
+    const uint64_t srcG = (uint64_t)__cvta_generic_to_global(has_g ? p.G : p.RX) + col_bytes + (g_rm ? (uint64_t)j0 * sizeof(S) : (uint64_t)0);
+    const bool g_ok = has_g && !(p.debug_mode & 4096);              // bit 12: no R_Y / G loads (timing probe)
+    const bool ry_ok = !(p.debug_mode & 4096);
+    const uint32_t ring_lane = smem_u32(ring) + (uint32_t)(t_lane * SEG + pc * 16);
+    const uint32_t *rw_lane = rw_s + sub * RW + t_lane;
+    const int a_lane = sub * RW + t_lane;
     auto issue_chunk = [&](int c) {
       if (c < nchunks) {
-        uint8_t *slot = ring + (c % FE_DEPTH) * FE_SLOT_BYTES;
+        const uint32_t d0 = ring_lane + (uint32_t)((c % FE_DEPTH) * FE_SLOT_BYTES);
 #pragma unroll
         for (int hsel = 0; hsel < 2; ++hsel) {
-          const int a = c * R + sub * RW + t_lane + RSTEP * hsel;
-          const uint32_t w = (a < p.n_loc && colok) ? rw_s[a] : 0u;
-          const bool valid = (a < p.n_loc) && colok && !(p.debug_mode & 2048);     // bit 11: no epilogue loads (timing probe)
-          const bool first = ((w >> 30) & 1u) && !(p.debug_mode & 4096);           // bit 12: no R_Y / G loads (timing probe)
-          const uint64_t off = (uint64_t)(w & 0x3FFFFFFFu) * (128 * sizeof(S)) + col_bytes;
-          uint8_t *d = slot + dst_lane + hsel * (RSTEP * SEG);
-          cp_async16(d, srcRX + off, valid ? 16u : 0u);
-          cp_async16(d + 1024, srcRY + off, (valid && first) ? 16u : 0u);
-          // G: panel layout like R_X / R_Y, or the caller's own row-major block (g_rowmajor)
-          const uint64_t offg = p.g_rowmajor ? ((uint64_t)((w & 0x3FFFFFFFu) - (uint32_t)(blockIdx.x * p.m)) * (uint64_t)p.N + j0) * sizeof(S) + col_bytes
-                                             : off;
-          cp_async16(d + 2048, (has_g ? srcG + offg : srcRX + off), (valid && first && has_g) ? 16u : 0u);
+          const uint32_t w = rw_lane[c * R + RSTEP * hsel];        // padded with zeros past n_loc
+          const bool valid = (c * R + RSTEP * hsel + a_lane < p.n_loc) && colok;
+          const bool first = (w & 0x40000000u) != 0;
+          const uint32_t rowp = w & 0x3FFFFFFFu;
+          const uint32_t d = d0 + hsel * (RSTEP * SEG);
+          cp_async16_sa(d, mad_wide_u32(rowp, ROWB, srcRX), valid ? 16u : 0u);
+          cp_async16_sa(d + 1024, mad_wide_u32(rowp, ROWB, srcRY), (valid && first && ry_ok) ? 16u : 0u);
+          cp_async16_sa(d + 2048, mad_wide_u32(rowp - g_sub, g_rowb, srcG), (valid && first && g_ok) ? 16u : 0u);
         }
       }
       cp_async_commit();
+    };
+    // rows of one chunk
+    auto do_rows = [&](int c, const uint32_t (&r)[RW]) {
+      const int a0 = c * R + sub * RW;
+      const int nv = do_store ? p.n_loc - a0 : 0;                   // rows t < nv are stored by this lane
+      const uint8_t *slot = ring + (c % FE_DEPTH) * FE_SLOT_BYTES;
+      const S *rxs = reinterpret_cast<const S *>(slot) + lane;
+      const S *rys = reinterpret_cast<const S *>(slot + 1024) + lane;
+      const S *gs = reinterpret_cast<const S *>(slot + 2048) + lane;
+      uint32_t wv[RW];
+      S rxv[RW], ryv[RW], gv[RW], Tv[RW];
+#pragma unroll
+      for (int q = 0; q < RW / 4; ++q) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(rw_s + a0 + 4 * q);
+        wv[4 * q] = v.x; wv[4 * q + 1] = v.y; wv[4 * q + 2] = v.z; wv[4 * q + 3] = v.w;
+      }
+#pragma unroll
+      for (int t = 0; t < RW; ++t) {
+        rxv[t] = rxs[t * 32];
+        ryv[t] = rys[t * 32];
+        gv[t] = gs[t * 32];
+        Tv[t] = (S)__uint_as_float(r[t]);
+      }
+      if (p.dinv_out) {                                             // ChFSI: D^-1 on the output rows
+#pragma unroll
+        for (int t = 0; t < RW; ++t)
+          if (a0 + t < p.n_loc) Tv[t] *= (S)p.dinv_out[(wv[t] & 0x3FFFFFFFu) - tile_m];
+      }
+      S outv[RW];
+#pragma unroll
+      for (int t = 0; t < RW; ++t) {
+        const uint32_t w = wv[t];
+        const S out_first = ka * Tv[t] + kb_ * ryv[t] + kc * rxv[t] + ka * (gv[t] * ly);
+        const S out_later = rxv[t] + ka * Tv[t];
+        outv[t] = (w & 0x40000000u) ? out_first : out_later;
+        if (t < nv) st_global(mad_wide_u32(w & 0x3FFFFFFFu, ROWB, rx_lane), outv[t]);
+      }
+      if (has_shadow) {                                             // last toucher: operand-precision shadow row
+#pragma unroll
+        for (int t = 0; t < RW; ++t) {
+          const uint32_t w = wv[t];
+          if (t < nv && (w & 0x80000000u)) {
+            if constexpr (KIND == 0) {
+              uint32_t u;
+              asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"((float)outv[t]));
+              st_global_u32(mad_wide_u32(w & 0x3FFFFFFFu, 128 * WB, wn_lane), u);
+            } else {
+              st_global_u16(mad_wide_u32(w & 0x3FFFFFFFu, 128 * WB, wn_lane), __bfloat16_as_ushort(__float2bfloat16_rn((float)outv[t])));
+            }
+          }
+        }
+      }
     };
     mbar_wait(accum_bar, 0);     // every MMA done: TMEM complete, operand stages free for the rings
     tc_fence_after();
     if (!(p.debug_mode & 4)) {
 #pragma unroll
       for (int c = 0; c < FE_DEPTH - 1; ++c) issue_chunk(c);
+      // accumulator columns of chunk c + 1 are requested while chunk c is processed
+      const uint32_t tm0 = tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(sub * RW);
+      uint32_t rn[RW];
+      if constexpr (RW == 8) tmem_ld_32x8(tm0, rn); else tmem_ld_32x4(tm0, rn);
 #pragma unroll 1
       for (int c = 0; c < nchunks; ++c) {
         issue_chunk(c + FE_DEPTH - 1);
-        uint32_t r[RW];
-        if constexpr (RW == 8)
-          tmem_ld_32x8(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(c * R + sub * RW), r);
-        else
-          tmem_ld_32x4(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(c * R + sub * RW), r);
         tmem_ld_wait();
+        uint32_t r[RW];
+#pragma unroll
+        for (int t = 0; t < RW; ++t) r[t] = rn[t];
+        if (c + 1 < nchunks) {
+          if constexpr (RW == 8) tmem_ld_32x8(tm0 + (uint32_t)((c + 1) * R), rn); else tmem_ld_32x4(tm0 + (uint32_t)((c + 1) * R), rn);
+        }
         cp_async_wait<FE_DEPTH - 1>();
         __syncwarp();
-        const uint8_t *slot = ring + (c % FE_DEPTH) * FE_SLOT_BYTES;
-        const S *rxs = reinterpret_cast<const S *>(slot);
-        const S *rys = reinterpret_cast<const S *>(slot + 1024);
-        const S *gs = reinterpret_cast<const S *>(slot + 2048);
-#pragma unroll
-        for (int t = 0; t < RW; ++t) {
-          const int a = c * R + sub * RW + t;
-          if (a < p.n_loc && jok) {
-            const uint32_t w = rw_s[a];
-            const uint32_t flt = w >> 30;
-            const int64_t idx = (int64_t)(w & 0x3FFFFFFFu) * 128 + jl;
-            S T = (S)__uint_as_float(r[t]);
-            if (p.dinv_out) T *= (S)p.dinv_out[(w & 0x3FFFFFFFu) - (uint32_t)(blockIdx.x * p.m)];
-            S out;
-            if (flt & 1u)
-              out = ka * T + kb_ * rys[t * 32 + lane] + kc * rxs[t * 32 + lane] + ka * (gs[t * 32 + lane] * ly);
-            else
-              out = rxs[t * 32 + lane] + ka * T;
-            if (!(p.debug_mode & 1024)) RX[idx] = out;                             // bit 10: no stores (timing probe)
-            if (p.Wnext && (flt & 2u) && !(p.debug_mode & 1024)) {
-              if constexpr (KIND == 0) {
-                uint32_t u;
-                asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"((float)out));
-                reinterpret_cast<uint32_t *>(p.Wnext)[idx] = u;
-              } else {
-                reinterpret_cast<__nv_bfloat16 *>(p.Wnext)[idx] = __float2bfloat16_rn((float)out);
-              }
-            }
-          }
-        }
+        do_rows(c, r);
         __syncwarp();     // all lanes done with this slot before it is refilled
       }
       cp_async_wait<0>();

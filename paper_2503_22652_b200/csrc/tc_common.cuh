@@ -109,6 +109,25 @@ __device__ __forceinline__ void tma_gather4(void *smem_dst, const CUtensorMap *m
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, uint32_t src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(src_bytes) : "memory");
 }
+// base + a * b with a 32 x 32 -> 64-bit multiply-add: one IMAD.WIDE instead of the shift / mask / carry chain the
+// compiler builds for (size_t)a * b + base
+__device__ __forceinline__ uint64_t mad_wide_u32(uint32_t a, uint32_t b, uint64_t base) {
+  uint64_t r;
+  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(base));
+  return r;
+}
+// global stores / cp.async sources addressed by a 64-bit integer (keeps the .global state space)
+__device__ __forceinline__ void st_global(uint64_t addr, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory"); }
+__device__ __forceinline__ void st_global(uint64_t addr, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(addr), "d"(v) : "memory"); }
+__device__ __forceinline__ void st_global_u32(uint64_t addr, uint32_t v) { asm volatile("st.global.u32 [%0], %1;" ::"l"(addr), "r"(v) : "memory"); }
+__device__ __forceinline__ void st_global_u16(uint64_t addr, uint16_t v) { asm volatile("st.global.u16 [%0], %1;" ::"l"(addr), "h"(v) : "memory"); }
+__device__ __forceinline__ void cp_async16_sa(uint32_t smem_dst, uint64_t gsrc, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
+}
+// the same with the destination given as a 32-bit shared-window address
+__device__ __forceinline__ void cp_async16_s(uint32_t smem_dst, const void *gsrc, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
+}
 // the mbarrier receives one arrival from this thread when all its earlier cp.async have landed
 // (.noinc: the arrival is part of the barrier's expected count)
 __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t *bar) {
