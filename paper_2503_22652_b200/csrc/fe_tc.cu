@@ -97,8 +97,6 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   const int npanels = (p.debug_mode & 512) ? 0 : (p.ksteps * KSTEP + KR - 1) / KR;   // bit 9: fixed-cost probe
   const uint32_t tmem_cols = (p.np <= 32) ? 32u : (p.np <= 64 ? 64u : (p.np <= 128 ? 128u : (p.np <= 256 ? 256u : 512u)));
 
-  for (int t = threadIdx.x; t < ((p.n_loc + 31) & ~31); t += blockDim.x)      // zero padded to whole chunks
-    rw_s[t] = t < p.n_loc ? ((uint32_t)(blockIdx.x * p.m + p.conn[cell * p.n_loc + t]) | ((uint32_t)p.flags[cell * p.n_loc + t] << 30)) : 0u;
   if (warp == FE_WORK_WARPS && lane == 0) {
     tma_prefetch_desc(&tmA);
     for (int s = 0; s < FE_STAGES; ++s) {
@@ -107,7 +105,17 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     }
     mbar_init(accum_bar, 1);
     fence_barrier_init();
+    // the first FE_STAGES cell-matrix panels need nothing from the other warps: their TMA loads go out before the
+    // node words are set up and TMEM is allocated, so ~1 us of the per-CTA fixed cost runs under their latency
+    for (int pn = 0; pn < min(FE_STAGES, npanels); ++pn) {
+      uint8_t *as = smem + pn * stage_bytes + FE_W_BYTES;
+      mbar_expect_tx(full_bar + pn, p.np * 128);
+      for (int hh = 0; hh < p.nh; ++hh)
+        tma_load_2d(as + hh * p.nhalf * 128, &tmA, full_bar + pn, 0, (int32_t)((cell * npanels + pn) * p.np + hh * p.nhalf));
+    }
   }
+  for (int t = threadIdx.x; t < ((p.n_loc + 31) & ~31); t += blockDim.x)      // zero padded to whole chunks
+    rw_s[t] = t < p.n_loc ? ((uint32_t)(blockIdx.x * p.m + p.conn[cell * p.n_loc + t]) | ((uint32_t)p.flags[cell * p.n_loc + t] << 30)) : 0u;
   if (warp == FE_WORK_WARPS + 1) tmem_alloc(tmem_slot, tmem_cols);
   tc_fence_before();
   __syncthreads();
@@ -116,8 +124,8 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   const bool has_g = p.G != nullptr;
 
   if (warp == FE_WORK_WARPS) {
-    // ===== TMA producer: cell-matrix panels =====
-    for (int pn = 0; pn < npanels; ++pn) {
+    // ===== TMA producer: cell-matrix panels (the first FE_STAGES were issued during the set-up) =====
+    for (int pn = FE_STAGES; pn < npanels; ++pn) {
       const int s = pn % FE_STAGES;
       mbar_wait(empty_bar + s, ((pn / FE_STAGES) & 1) ^ 1);
       if (elect_one()) {
