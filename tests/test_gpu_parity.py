@@ -530,9 +530,11 @@ def test_chunked_rayleigh_ritz_matches_oracle_and_full_variant(monkeypatch):
         s.close()
 
 
-def test_memory_light_solve_keeps_fp32_residual_block(monkeypatch):
+@pytest.mark.parametrize("apply_prec", ["tf32", "bf16"])
+def test_memory_light_solve_keeps_fp32_residual_block(monkeypatch, apply_prec):
     """rchfsi_solve in the memory-light mode (chunked Rayleigh-Ritz + FP32 G read in place by the fused steps):
-    still converges to the exact eigenvalues with residual <= 1e-8."""
+    still converges to the exact eigenvalues with residual <= 1e-8.  bf16 is the config-5 scheme as
+    BASELINE.json states it: BF16 cell-GEMM operands through the one shadow block updated in place."""
     torch = _torch()
     import scipy.linalg as sla
     import paper_2503_22652_b200 as P
@@ -545,7 +547,7 @@ def test_memory_light_solve_keeps_fp32_residual_block(monkeypatch):
     N, nw, p = 16, 8, 30
     X0 = np.random.default_rng(2).standard_normal((m, N))
     As, Bs, dinv = P.upload_problem(prob)
-    sol = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec="tf32", store_prec="fp32", adaptive_bounds=True)
+    sol = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec=apply_prec, store_prec="fp32", adaptive_bounds=True)
     out = sol.solve(P.METHOD_RCHFSI, torch.as_tensor(X0).cuda(), nw, p, ev[0] - 1.0, ev[N], lam_max, tol=1e-8, max_iter=80)
     assert out["converged"], out["history"][-5:]
     np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8, atol=1e-9)
