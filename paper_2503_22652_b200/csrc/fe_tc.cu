@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     // node words are set up and TMEM is allocated, so ~1 us of the per-CTA fixed cost runs under their latency
     for (int pn = 0; pn < min(FE_STAGES, npanels); ++pn) {
       uint8_t *as = smem + pn * stage_bytes + FE_W_BYTES;
+      if (p.debug_mode & 8192) { mbar_arrive(full_bar + pn); continue; }    // bit 13: MMA-only probe (no TMA, no gather reads)
       mbar_expect_tx(full_bar + pn, p.np * 128);
       for (int hh = 0; hh < p.nh; ++hh)
         tma_load_2d(as + hh * p.nhalf * 128, &tmA, full_bar + pn, 0, (int32_t)((cell * npanels + pn) * p.np + hh * p.nhalf));
@@ -130,9 +131,13 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
       mbar_wait(empty_bar + s, ((pn / FE_STAGES) & 1) ^ 1);
       if (elect_one()) {
         uint8_t *as = smem + s * stage_bytes + FE_W_BYTES;
-        mbar_expect_tx(full_bar + s, p.np * 128);
-        for (int hh = 0; hh < p.nh; ++hh)
-          tma_load_2d(as + hh * p.nhalf * 128, &tmA, full_bar + s, 0, (int32_t)((cell * npanels + pn) * p.np + hh * p.nhalf));
+        if (p.debug_mode & 8192) {
+          mbar_arrive(full_bar + s);
+        } else {
+          mbar_expect_tx(full_bar + s, p.np * 128);
+          for (int hh = 0; hh < p.nh; ++hh)
+            tma_load_2d(as + hh * p.nhalf * 128, &tmA, full_bar + s, 0, (int32_t)((cell * npanels + pn) * p.np + hh * p.nhalf));
+        }
       }
       __syncwarp();
     }
@@ -191,7 +196,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
           }
           const int kk = pn * KR + k;
           const int cl = (a * 128 + c16 * 16) / EB;     // column inside the 128-column panel
-          const bool ok = kk < p.n_loc && j0 + cl < p.N;
+          const bool ok = kk < p.n_loc && j0 + cl < p.N && !(p.debug_mode & 8192);
           const uint32_t rowp = ok ? (rw_s[kk] & 0x3FFFFFFFu) : 0u;
           // panel layout [column tile][m][128]: the rows of one tile are 128 * EB bytes apart
           cp_async16(ws + dst_off, Wb + ((uint64_t)rowp * 128 + (ok ? cl : 0)) * EB, ok ? 16u : 0u);
