@@ -71,7 +71,9 @@ typedef enum { RCHFSI_METHOD_CHFSI = 0, RCHFSI_METHOD_RCHFSI = 1 } rchfsi_method
  *         cell_mats is [n_cells][n_loc][n_loc], or ONE [n_loc][n_loc] matrix shared by
  *         every cell when cell_shared != 0.  Every cell matrix must be symmetric (it is
  *         the element matrix of a symmetric form; A is Hermitian): the
- *         kernels read A_c[b][a] for A_c[a][b].  rchfsi_create verifies this.
+ *         kernels read A_c[b][a] for A_c[a][b].  rchfsi_create verifies this, and that
+ *         every row 0..m-1 occurs in conn (EINVAL otherwise: a row no cell touches has
+ *         no place in the coloured scatter).
  *         cell_mats_f32, if non-NULL, is the same array in FP32 and may be given INSTEAD
  *         of cell_mats (cell_mats == NULL) when the FP64 copy does not fit (config 5:
  *         13 GB); it is then also what the FP64 Rayleigh-Ritz path reads (widened). */
@@ -104,8 +106,6 @@ typedef struct {
                                  T_j += eps ||T_j|| g_j/||g_j|| inside the filter only
                                  (BASELINE.json configs[0]; reading S11) */
   uint64_t noise_seed;
-  int32_t use_cuda_graph;     /* reserved (ignored): the step coefficients are kernel arguments, so a graph
-                                 would have to be re-captured per call; measured launch gaps are < 2 us */
   int32_t g_input_f32;        /* nonzero: the G argument of rchfsi_filter points to FP32 values [m][N] (an FP64
                                  residual block does not fit at config 5, SURVEY 8(d) memory plan); needs
                                  store_prec FP32; G is then read in place, no copy is made */
@@ -128,6 +128,13 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A,
                             int32_t block_N, const rchfsi_options *opt, void *cuda_stream);
 
 rchfsi_status rchfsi_destroy(rchfsi_handle h);
+
+/* The CONTENTS of the operator arrays and of dinv_diag are borrowed too: the filter keeps reduced-precision
+ * copies of A (with D^-1 folded in) that are built on first use.  When the caller updates A or dinv_diag in
+ * place (the A of an SCF iteration evolves), call this before the next filter: it synchronises
+ * the stream and drops the copies so that they are rebuilt.  The sparsity pattern / connectivity must not
+ * change (make a new handle for that). */
+rchfsi_status rchfsi_operator_changed(rchfsi_handle h);
 
 /* Message for the most recent failure on this handle ("" if none); NULL handle => the
  * message of the last failed rchfsi_create in this thread. */
@@ -159,7 +166,8 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
                             double lam_max);
 
 /* Same call with HOST buffers: copies X, ritz (and G if non-NULL) to device scratch,
- * runs rchfsi_filter, copies Y_p back into X_host, synchronises. */
+ * runs rchfsi_filter, copies Y_p back into X_host, synchronises.  G_host holds FP64 values,
+ * or FP32 values when the handle was created with g_input_f32. */
 rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host,
                                  const double *ritz_host, const double *G_host,
                                  int32_t degree, double lam_min, double lam_T, double lam_max);

@@ -29,7 +29,7 @@ class RchfsiOptions(C.Structure):
     _fields_ = [("apply_prec", C.c_int32), ("store_prec", C.c_int32),
                 ("normalize_columns_before_rr", C.c_int32), ("adaptive_bounds", C.c_int32),
                 ("noise_eps", C.c_double), ("noise_seed", C.c_uint64),
-                ("use_cuda_graph", C.c_int32), ("g_input_f32", C.c_int32)]
+                ("g_input_f32", C.c_int32)]
 
 
 # every symbol include/rchfsi.h declares: name -> (restype, argtypes)
@@ -39,6 +39,7 @@ SYMBOLS = {
     "rchfsi_create": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(RchfsiOperator), C.POINTER(RchfsiOperator),
                                 C.c_void_p, C.c_int32, C.POINTER(RchfsiOptions), C.c_void_p]),
     "rchfsi_destroy": (C.c_int, [C.c_void_p]),
+    "rchfsi_operator_changed": (C.c_int, [C.c_void_p]),
     "rchfsi_last_error": (C.c_char_p, [C.c_void_p]),
     "rchfsi_workspace_bytes": (C.c_size_t, [C.POINTER(RchfsiOperator), C.POINTER(RchfsiOperator), C.c_int32,
                                             C.POINTER(RchfsiOptions)]),
@@ -136,7 +137,7 @@ class Rchfsi:
 
     def __init__(self, A, B=None, dinv=None, block_N=1, apply_prec="fp64", store_prec="fp64",
                  normalize_columns_before_rr=True, adaptive_bounds=False, noise_eps=0.0, noise_seed=0,
-                 use_cuda_graph=False, g_input_f32=False, stream=None):
+                 g_input_f32=False, stream=None):
         import torch
         self.lib = load_library()
         self._keep = []
@@ -152,7 +153,6 @@ class Rchfsi:
         opt.adaptive_bounds = int(adaptive_bounds)
         opt.noise_eps = float(noise_eps)
         opt.noise_seed = int(noise_seed)
-        opt.use_cuda_graph = int(use_cuda_graph)
         opt.g_input_f32 = int(g_input_f32)
         self.opt = opt
         self.m, self.N = int(self.opA.m), int(block_N)
@@ -178,6 +178,12 @@ class Rchfsi:
             self.close()
         except Exception:
             pass
+
+    def operator_changed(self):
+        """rchfsi_operator_changed: the caller rewrote A / dinv in place; drop the reduced-precision copies."""
+        st = self.lib.rchfsi_operator_changed(self.h)
+        if st != OK:
+            self._raise(st)
 
     def _block(self, t, name):
         import torch
@@ -207,11 +213,27 @@ class Rchfsi:
     def filter_host(self, method, X_host, ritz_host, G_host, degree, lam_min, lam_T, lam_max):
         """rchfsi_filter_host: numpy / CPU-tensor buffers (float64, C-contiguous); X_host is
         overwritten with Y_p.  Host<->device copies happen inside the call."""
-        def hp(a):
+        import numpy as np
+
+        def hp(a, name, shape, f32=False):
             if a is None:
                 return C.c_void_p(0)
-            return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
-        st = self.lib.rchfsi_filter_host(self.h, method, hp(X_host), hp(ritz_host), hp(G_host), degree,
+            if hasattr(a, "data_ptr"):      # CPU torch tensor
+                import torch
+                ok = (not a.is_cuda and a.is_contiguous() and tuple(a.shape) == shape
+                      and a.dtype == (torch.float32 if f32 else torch.float64))
+                ptr = a.data_ptr()
+            else:
+                ok = (isinstance(a, np.ndarray) and a.flags["C_CONTIGUOUS"] and a.shape == shape
+                      and a.dtype == (np.float32 if f32 else np.float64))
+                ptr = a.ctypes.data if ok else 0
+            if not ok:
+                raise TypeError("%s must be a C-contiguous host array of shape %s, %s" %
+                                (name, shape, "float32" if f32 else "float64"))
+            return C.c_void_p(ptr)
+        blk = (self.m, self.N)
+        st = self.lib.rchfsi_filter_host(self.h, method, hp(X_host, "X_host", blk), hp(ritz_host, "ritz_host", (self.N,)),
+                                         hp(G_host, "G_host", blk, f32=bool(self.opt.g_input_f32)), degree,
                                          lam_min, lam_T, lam_max)
         if st != OK:
             self._raise(st)

@@ -2,6 +2,7 @@
 // host-side control flow of Algorithms 1-3.  All arithmetic on blocks
 // runs in the CUDA kernels of this library; the host only computes the Chebyshev scalars.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include "common.cuh"
 
@@ -58,6 +59,28 @@ static bool operator_ok(const rchfsi_operator *op, std::string &why) {
   }
 }
 
+// the environment is read here, once per handle, never on the per-step launch path
+static Knobs read_knobs() {
+  Knobs k;
+  auto geti = [](const char *name, int dflt) {
+    const char *e = getenv(name);
+    return e ? atoi(e) : dflt;
+  };
+  k.fe_shadow_pair = getenv("RCHFSI_FE_SHADOW_PAIR") != nullptr;
+  k.fe_legacy = geti("RCHFSI_FE_LEGACY", 0) != 0;
+  k.dense_bn = geti("RCHFSI_DENSE_BN", 0);
+  k.dense_ks = geti("RCHFSI_DENSE_KS", 0);
+  k.dense_mc = geti("RCHFSI_DENSE_MC", -1);
+  k.rr_chunked = geti("RCHFSI_RR_CHUNKED", -1);
+  k.rr_fe_simt = getenv("RCHFSI_RR_FE_SIMT") != nullptr;
+  k.rr_timing = getenv("RCHFSI_RR_TIMING") != nullptr;
+  k.rr_split = geti("RCHFSI_RR_SPLIT", -1);
+#ifdef RCHFSI_PROBES
+  k.tc_debug = geti("RCHFSI_TC_DEBUG", 0);
+#endif
+  return k;
+}
+
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const rchfsi_operator *B,
@@ -90,8 +113,10 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const 
   h->dinv = dinv_diag;
   h->m = A->m;
   h->N = block_N;
+  h->N_cap = block_N;
   h->opt = o;
   h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  h->knobs = read_knobs();
   for (const rchfsi_operator *op : {A, B}) {
     if (op && op->kind == RCHFSI_OP_FE) {
       double asym = 0.0;
@@ -103,6 +128,11 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const 
         return RCHFSI_EINVAL;
       }
     }
+  }
+  if (A->kind == RCHFSI_OP_FE) {
+    // colouring of the cell conflict graph; also validates conn (range, every row covered by a cell)
+    rchfsi_status s = fe_ensure_coloring(h);
+    if (s != RCHFSI_OK) { g_create_error = h->err; rchfsi_destroy(h); return s; }
   }
   if (cudaEventCreate(&h->ev_step0) != cudaSuccess || cudaEventCreate(&h->ev_step1) != cudaSuccess) {
     g_create_error = "cudaEventCreate failed";
@@ -119,11 +149,28 @@ rchfsi_status rchfsi_destroy(rchfsi_handle h) {
   for (void *p : h->owned) cudaFree(p);
   if (h->cublas) cublasDestroy(h->cublas);
   if (h->cusolver) cusolverDnDestroy(h->cusolver);
-  if (h->ev_x) cudaEventDestroy(h->ev_x);
-  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  for (int i = 0; i < rchfsi_ctx::HOST_SETS; ++i)
+    for (cudaEvent_t e : {h->ev_g[i], h->ev_xin[i], h->ev_done[i], h->ev_free[i]})
+      if (e) cudaEventDestroy(e);
+  if (h->in_stream) cudaStreamDestroy(h->in_stream);
+  if (h->out_stream) cudaStreamDestroy(h->out_stream);
   if (h->ev_step0) cudaEventDestroy(h->ev_step0);
   if (h->ev_step1) cudaEventDestroy(h->ev_step1);
   delete h;
+  return RCHFSI_OK;
+}
+
+rchfsi_status rchfsi_operator_changed(rchfsi_handle h) {
+  if (!h) return RCHFSI_EINVAL;
+  RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(h->stream));
+  // the reduced-precision copies (with D^-1 folded in) and the TMA descriptors onto them are rebuilt on the next step
+  for (rchfsi::LowpCopy &c : h->lowp) {
+    for (size_t i = 0; i < h->owned.size(); ++i)
+      if (h->owned[i] == c.data) { h->owned.erase(h->owned.begin() + i); break; }
+    cudaFree(c.data);
+  }
+  h->lowp.clear();
+  h->tmaps.clear();
   return RCHFSI_OK;
 }
 

@@ -7,9 +7,18 @@
 #include <cublas_v2.h>
 #include <cusolverDn.h>
 #include <stdint.h>
+#include <map>
 #include <string>
 #include <vector>
 #include "rchfsi.h"
+
+// Timing probes that switch parts of the tensor-core kernels off (RCHFSI_TC_DEBUG) exist only in builds
+// with -DRCHFSI_PROBES; the shipped library compiles them out (PROBE folds to 0).
+#ifdef RCHFSI_PROBES
+#define PROBE(mode, bits) ((mode) & (bits))
+#else
+#define PROBE(mode, bits) 0
+#endif
 
 namespace rchfsi {
 
@@ -38,6 +47,20 @@ struct TmapEntry {
   CUtensorMap map;
 };
 
+// Test / tuning knobs, read from the environment ONCE in rchfsi_create (never on the per-step launch path).
+struct Knobs {
+  bool fe_shadow_pair = false;   // RCHFSI_FE_SHADOW_PAIR: two operand-shadow buffers instead of the in-place one
+  bool fe_legacy = false;        // RCHFSI_FE_LEGACY: the one-tile-per-CTA FE kernel also for BF16 (A/B against the pipelined one)
+  int dense_bn = 0;              // RCHFSI_DENSE_BN: 64 / 128 / 256, 0 = automatic
+  int dense_ks = 0;              // RCHFSI_DENSE_KS: K splits 1 / 2 / 4 / 8, 0 = automatic
+  int dense_mc = -1;             // RCHFSI_DENSE_MC: operator-tile multicast on / off, -1 = automatic
+  int rr_chunked = -1;           // RCHFSI_RR_CHUNKED: force the memory-light Rayleigh-Ritz on / off
+  bool rr_fe_simt = false;       // RCHFSI_RR_FE_SIMT: FE applies of the Rayleigh-Ritz through the hand-written FP64 kernel
+  bool rr_timing = false;        // RCHFSI_RR_TIMING: print phase times of the Rayleigh-Ritz to stderr
+  int rr_split = -1;             // RCHFSI_RR_SPLIT: Gram / rotation products on the tensor pipe (split operands), -1 = automatic
+  int tc_debug = 0;              // RCHFSI_TC_DEBUG (only in -DRCHFSI_PROBES builds)
+};
+
 struct DeviceOperator {
   rchfsi_operator d{};    // caller's descriptor (device pointers, borrowed)
   bool present = false;
@@ -57,7 +80,8 @@ struct rchfsi_ctx {
   rchfsi::DeviceOperator A, B;
   const double *dinv = nullptr;
   int64_t m = 0;
-  int32_t N = 0;
+  int32_t N = 0;        // ACTIVE block width of the current call (= N_cap except inside a column chunk of filter_host)
+  int32_t N_cap = 0;    // block width the handle was created for: every workspace block is sized for it
   rchfsi_options opt{};
   cudaStream_t stream = nullptr;
   cublasHandle_t cublas = nullptr;
@@ -76,6 +100,8 @@ struct rchfsi_ctx {
   double *colnorm = nullptr;              // [2][N]
   std::vector<rchfsi::LowpCopy> lowp;
   std::vector<rchfsi::TmapEntry> tmaps;
+  rchfsi::Knobs knobs;
+  std::map<const void *, int> func_smem;   // per handle (= per device): dynamic shared memory opted in per kernel
   rchfsi::FeColoring coloring;
 
   // Rayleigh-Ritz workspace
@@ -90,11 +116,18 @@ struct rchfsi_ctx {
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
 
-  // host-buffer entry point scratch; the H2D copy of X runs on copy_stream behind the recurrence (Alg. 3 reads X
-  // only in its last line) and the main stream waits for ev_x before the finish kernel
-  double *hX = nullptr, *hG = nullptr, *hritz = nullptr;
-  cudaStream_t copy_stream = nullptr;
-  cudaEvent_t ev_x = nullptr;
+  // host-buffer entry point (rchfsi_filter_host): column chunks of the block travel host -> device on in_stream,
+  // are filtered on the main stream and return on out_stream, three staging sets in rotation.  Alg. 3 reads X only
+  // in its last line, so the main stream waits for the chunk's X (ev_x) only before the finish kernel.
+  static constexpr int HOST_SETS = 3;
+  double *hX[HOST_SETS] = {nullptr, nullptr, nullptr};
+  void *hG[HOST_SETS] = {nullptr, nullptr, nullptr};
+  double *hritz = nullptr;
+  int32_t host_chunk = 0;                  // staging width (columns) the sets were allocated for
+  cudaStream_t in_stream = nullptr, out_stream = nullptr;
+  cudaEvent_t ev_g[HOST_SETS] = {nullptr, nullptr, nullptr}, ev_xin[HOST_SETS] = {nullptr, nullptr, nullptr},
+              ev_done[HOST_SETS] = {nullptr, nullptr, nullptr}, ev_free[HOST_SETS] = {nullptr, nullptr, nullptr};
+  cudaEvent_t ev_x = nullptr;              // the X event the running filter has to wait for (one of ev_xin)
   bool x_pending = false;
 
   // instrumentation
@@ -122,6 +155,8 @@ namespace rchfsi {
   } while (0)
 
 rchfsi_status dev_alloc(rchfsi_ctx *h, void **p, size_t bytes);
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (handle, kernel)
+rchfsi_status ensure_func_smem(rchfsi_ctx *h, const void *func, int bytes);
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 #define LAUNCH_CHECK(h)                                                                   \
@@ -176,9 +211,6 @@ rchfsi_status chfsi_first(rchfsi_ctx *h, int store_prec, int t_prec, int shadow_
 // RCHFSI finish: X = dinv * RY + X * LY (PAPER.md:263 last line); CHFSI finish: X = RY
 rchfsi_status finish_block(rchfsi_ctx *h, int store_prec, const void *RY, const double *dinv,
                            const double *LY, double *X, int64_t m, int32_t N, int64_t pm = 0);
-// FP64 -> operand precision shadow of X (CHFSI start)
-rchfsi_status convert_block(rchfsi_ctx *h, int dst_prec, const double *src, void *dst, int64_t m,
-                            int32_t N);
 // column 2-norms (sum of squares accumulated in FP64 with atomics into a zeroed array)
 rchfsi_status column_sumsq(rchfsi_ctx *h, int prec, const void *V, int64_t m, int32_t N,
                            double *sumsq);

@@ -45,17 +45,28 @@ bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16,
   return r == CUDA_SUCCESS;
 }
 
-const CUtensorMap *get_tmap_2d(rchfsi_ctx *h, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
-                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32) {
+bool get_tmap_2d(rchfsi_ctx *h, CUtensorMap *out, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
+                 uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32) {
   for (const TmapEntry &e : h->tmaps)
     if (e.base == base && e.rows == rows && e.cols == cols && e.pitch == pitch_bytes && e.box_cols == box_cols &&
-        e.box_rows == box_rows && e.elem_bytes == elem_bytes && e.bf16 == (int)bf16 && e.atom32 == (int)atom32)
-      return &e.map;
+        e.box_rows == box_rows && e.elem_bytes == elem_bytes && e.bf16 == (int)bf16 && e.atom32 == (int)atom32) {
+      *out = e.map;
+      return true;
+    }
   TmapEntry e{base, rows, cols, pitch_bytes, box_cols, box_rows, elem_bytes, (int)bf16, (int)atom32, {}};
-  if (!make_tmap_2d(&e.map, base, elem_bytes, bf16, rows, cols, pitch_bytes, box_cols, box_rows, atom32)) return nullptr;
-  if (h->tmaps.size() > 64) h->tmaps.clear();
+  if (!make_tmap_2d(&e.map, base, elem_bytes, bf16, rows, cols, pitch_bytes, box_cols, box_rows, atom32)) return false;
+  if (h->tmaps.size() >= 64) h->tmaps.erase(h->tmaps.begin());   // callers hold copies, never pointers into the cache
   h->tmaps.push_back(e);
-  return &h->tmaps.back().map;
+  *out = e.map;
+  return true;
+}
+
+rchfsi_status ensure_func_smem(rchfsi_ctx *h, const void *func, int bytes) {
+  auto it = h->func_smem.find(func);
+  if (it != h->func_smem.end() && it->second >= bytes) return RCHFSI_OK;
+  RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  h->func_smem[func] = bytes;
+  return RCHFSI_OK;
 }
 
 namespace {
@@ -148,7 +159,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       const uint32_t ph = (kb / Cfg::STAGES) & 1;
       mbar_wait(empty_bar + s, ph ^ 1);
       if (elect_one()) {
-        if (p.debug_mode & 2) {
+        if (PROBE(p.debug_mode, 2)) {
           mbar_arrive(full_bar + s);
         } else {
           mbar_expect_tx(full_bar + s, Cfg::STAGE_BYTES);
@@ -188,7 +199,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       mbar_wait(full_bar + s, ph);
       tc_fence_after();
       if (elect_one()) {
-        if (p.debug_mode & 1) {
+        if (PROBE(p.debug_mode, 1)) {
           mbar_arrive(empty_bar + s);
         } else {
 #pragma unroll
@@ -208,7 +219,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       __syncwarp();
     }
     if (elect_one()) {
-      if (p.debug_mode & 1) mbar_arrive(accum_bar); else umma_commit(accum_bar);
+      if (PROBE(p.debug_mode, 1)) mbar_arrive(accum_bar); else umma_commit(accum_bar);
     }
   }
   __syncwarp();
@@ -235,7 +246,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       float *part = reinterpret_cast<float *>(smem);
       const int jl = threadIdx.x & 127;
       const int jj = j0 + jl;
-      const bool jjok = jj < p.N && !(p.debug_mode & 4);
+      const bool jjok = jj < p.N && !PROBE(p.debug_mode, 4);
       const S ly2 = (S)((G != nullptr && jjok) ? p.LY[jj] : 0.0);
       const int cpr = BN / ks;                                  // matrix rows owned by this CTA
       const int cbase = blockIdx.z * cpr + (threadIdx.x >> 7);  // this thread: every second owned row
@@ -274,7 +285,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
         for (int t = 0; t < RB; ++t) T[t] = 0.f;
         // all the partial sums of the batch are requested before the first is used (fixed rank order: deterministic)
         for (int rr = 0; rr < ks; ++rr) {
-          const uint32_t base = dsmem_map(part_s, ((p.debug_mode & 64) ? blockIdx.z : (uint32_t)rr) * (mc ? 2u : 1u) + cx);   // bit 6: local reads only (timing probe)
+          const uint32_t base = dsmem_map(part_s, (PROBE(p.debug_mode, 64) ? blockIdx.z : (uint32_t)rr) * (mc ? 2u : 1u) + cx);   // bit 6: local reads only (timing probe)
           float pv[RB];
 #pragma unroll
           for (int t = 0; t < RB; ++t) {
@@ -314,7 +325,7 @@ __global__ void __launch_bounds__(256, 1) dense_tc_kernel(const __grid_constant_
       uint32_t r[32];
       tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)c0, r);
       tmem_ld_wait();
-      if (!jok || (p.debug_mode & 4)) continue;
+      if (!jok || PROBE(p.debug_mode, 4)) continue;
 #pragma unroll
       for (int t0 = 0; t0 < 32; t0 += 8) {
         S ry[8], rx[8], g[8];
@@ -409,11 +420,7 @@ rchfsi_status launch_dense(rchfsi_ctx *h, const CUtensorMap &tmW, const CUtensor
                            const DenseTcParams &p) {
   using Cfg = DenseCfg<BN>;
   auto kern = dense_tc_kernel<KIND, BN, S>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    RCHFSI_CUDA_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
-    attr_set = true;
-  }
+  RCHFSI_TRY(ensure_func_smem(h, reinterpret_cast<const void *>(kern), Cfg::SMEM_BYTES));
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3((unsigned)cdiv(p.N, 128), (unsigned)cdiv(p.m, BN), (unsigned)p.ksplit);
   cfg.blockDim = dim3(256);
@@ -453,12 +460,9 @@ bool dense_tc_supported(const rchfsi_ctx *h) {
 // over a 2-CTA cluster and the partial tiles summed through distributed shared memory -- 128 CTAs with an N = 128
 // MMA (96 cycles for twice the work of the 80-cycle N = 64 one) and 2/3 of the operand traffic of 64-row tiles;
 // measured 33.1 against 35.2 us per step.  Small problems: 64-row tiles.
-void dense_tc_pick(int64_t m, int32_t N, int nkb128, int *bn_out, int *ks_out) {
+void dense_tc_pick(const Knobs &kn, int64_t m, int32_t N, int nkb128, int *bn_out, int *ks_out) {
   int bn = 0, ks = 1;
-  if (const char *e = getenv("RCHFSI_DENSE_BN")) {   // tuning knobs
-    const int v = atoi(e);
-    if (v == 64 || v == 128 || v == 256) bn = v;
-  }
+  if (kn.dense_bn == 64 || kn.dense_bn == 128 || kn.dense_bn == 256) bn = kn.dense_bn;   // tuning knob
   const int64_t tj = cdiv(N, 128);
   if (bn == 0) {
     const int64_t t128 = tj * cdiv(m, 128);
@@ -467,10 +471,7 @@ void dense_tc_pick(int64_t m, int32_t N, int nkb128, int *bn_out, int *ks_out) {
     else if (2 * t128 >= 100 && 2 * t128 <= 148 && nkb128 >= 8) { bn = 128; ks = 2; }
     else bn = 64;
   }
-  if (const char *e = getenv("RCHFSI_DENSE_KS")) {
-    const int v = atoi(e);
-    if (v == 1 || v == 2 || v == 4 || v == 8) ks = v;
-  }
+  if (kn.dense_ks == 1 || kn.dense_ks == 2 || kn.dense_ks == 4 || kn.dense_ks == 8) ks = kn.dense_ks;
   *bn_out = bn;
   *ks_out = ks;
 }
@@ -484,25 +485,24 @@ rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
   const int eb = bf16 ? 2 : 4;
   const int32_t nkb = (int32_t)cdiv(h->m, (bf16 ? 64 : 32) * 2);
   int bn = 64, ks = 1;
-  dense_tc_pick(h->m, h->N, nkb, &bn, &ks);
+  dense_tc_pick(h->knobs, h->m, h->N, nkb, &bn, &ks);
   while (ks > 1 && (nkb < 2 * ks || bn % (2 * ks) != 0)) ks /= 2;
   // W [m][N]: box = 128 B of block columns x (32 | 64) k rows
-  const CUtensorMap *ptW = get_tmap_2d(h, s.W, eb, bf16, (uint64_t)h->m, (uint64_t)h->N, (uint64_t)h->N * eb,
-                                       bf16 ? 64 : 32, bf16 ? 64 : 32, !bf16);
-  const CUtensorMap *ptA = get_tmap_2d(h, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb,
-                                       bf16 ? 64 : 32, (uint32_t)bn);
-  // half-height operator tile for the multicast pair (each CTA fetches one half for both)
-  const CUtensorMap *ptAh = get_tmap_2d(h, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb,
-                                        bf16 ? 64 : 32, (uint32_t)bn / 2);
-  if (!ptW || !ptA || !ptAh) {
+  CUtensorMap tmW, tmA, tmAh;
+  // tmAh: half-height operator tile for the multicast pair (each CTA fetches one half for both)
+  if (!get_tmap_2d(h, &tmW, s.W, eb, bf16, (uint64_t)h->m, (uint64_t)h->N, (uint64_t)h->N * eb, bf16 ? 64 : 32,
+                   bf16 ? 64 : 32, !bf16) ||
+      !get_tmap_2d(h, &tmA, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb, bf16 ? 64 : 32,
+                   (uint32_t)bn) ||
+      !get_tmap_2d(h, &tmAh, cp->data, eb, bf16, (uint64_t)h->m, (uint64_t)cp->ld, (uint64_t)cp->ld * eb, bf16 ? 64 : 32,
+                   (uint32_t)bn / 2)) {
     h->err = "cuTensorMapEncodeTiled failed";
     return RCHFSI_ECUDA;
   }
-  const CUtensorMap tmW = *ptW, tmA = *ptA, tmAh = *ptAh;
   int mcast = (cdiv(h->N, 128) % 2 == 0 && 2 * ks <= 8) ? 1 : 0;
-  if (const char *e = getenv("RCHFSI_DENSE_MC")) mcast = mcast && atoi(e) != 0;   // tuning knob
-  const int dbg = getenv("RCHFSI_TC_DEBUG") ? atoi(getenv("RCHFSI_TC_DEBUG")) : 0;
-  if (dbg & 3) mcast = 0;                                                          // the timing probes assume one consumer per stage
+  if (h->knobs.dense_mc == 0) mcast = 0;                                           // tuning knob
+  const int dbg = h->knobs.tc_debug;
+  if (PROBE(dbg, 3)) mcast = 0;                                                    // the timing probes assume one consumer per stage
   DenseTcParams p{s.k, s.RY, s.RX, s.G, s.LY, s.chfsi ? h->dinv : nullptr, s.Wnext, h->m, h->N,
                   nkb, ks, mcast, dbg};
   if (s.store_prec == RCHFSI_FP64)

@@ -193,10 +193,6 @@ rchfsi_status finish_block(rchfsi_ctx *h, int store_prec, const void *RY, const 
                            const double *LY, double *X, int64_t m, int32_t N, int64_t pm) {
   return launch_misc(h, LY ? 2 : 3, 0.0, 0.0, RY, store_prec, dinv, LY, nullptr, X, RCHFSI_FP64, nullptr, 0, m, N, pm);
 }
-rchfsi_status convert_block(rchfsi_ctx *h, int dst_prec, const double *src, void *dst, int64_t m,
-                            int32_t N) {
-  return launch_misc(h, 0, 1.0, 0.0, nullptr, 0, nullptr, nullptr, src, dst, dst_prec, nullptr, 0, m, N);
-}
 
 // Lambda_k = C_k(Lambda), eq. (12): one thread per column, k sequential.
 __global__ void lambda_table_kernel(const double *__restrict__ ritz, int32_t N, int32_t p, double e,

@@ -88,7 +88,7 @@ __global__ void feg_pointers_kernel(const double **ptrs, int64_t batch, int64_t 
 }  // namespace
 
 bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op) {
-  if (getenv("RCHFSI_RR_FE_SIMT")) return false;                       // A/B knob: keep the hand-written kernel
+  if (h->knobs.rr_fe_simt) return false;                               // A/B knob: keep the hand-written kernel
   const rchfsi_operator &A = h->A.d;
   return op.kind == RCHFSI_OP_FE && A.kind == RCHFSI_OP_FE && op.conn == A.conn && op.n_cells == A.n_cells &&
          op.n_loc == A.n_loc && h->cublas != nullptr && (op.cell_mats != nullptr || op.cell_mats_f32 != nullptr);

@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
   const int lane = threadIdx.x & 31;
   const int j0 = blockIdx.x * 128;
   const int64_t cell = p.cell_order[blockIdx.y];
-  const int npanels = (p.debug_mode & 512) ? 0 : (p.ksteps * KSTEP + KR - 1) / KR;   // bit 9: fixed-cost probe
+  const int npanels = PROBE(p.debug_mode, 512) ? 0 : (p.ksteps * KSTEP + KR - 1) / KR;   // bit 9: fixed-cost probe
   const uint32_t tmem_cols = (p.np <= 32) ? 32u : (p.np <= 64 ? 64u : (p.np <= 128 ? 128u : (p.np <= 256 ? 256u : 512u)));
 
   if (warp == FE_WORK_WARPS && lane == 0) {
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     // node words are set up and TMEM is allocated, so ~1 us of the per-CTA fixed cost runs under their latency
     for (int pn = 0; pn < min(FE_STAGES, npanels); ++pn) {
       uint8_t *as = smem + pn * stage_bytes + FE_W_BYTES;
-      if (p.debug_mode & 8192) { mbar_arrive(full_bar + pn); continue; }    // bit 13: MMA-only probe (no TMA, no gather reads)
+      if (PROBE(p.debug_mode, 8192)) { mbar_arrive(full_bar + pn); continue; }    // bit 13: MMA-only probe (no TMA, no gather reads)
       mbar_expect_tx(full_bar + pn, p.np * 128);
       for (int hh = 0; hh < p.nh; ++hh)
         tma_load_2d(as + hh * p.nhalf * 128, &tmA, full_bar + pn, 0, (int32_t)((cell * npanels + pn) * p.np + hh * p.nhalf));
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
       mbar_wait(empty_bar + s, ((pn / FE_STAGES) & 1) ^ 1);
       if (elect_one()) {
         uint8_t *as = smem + s * stage_bytes + FE_W_BYTES;
-        if (p.debug_mode & 8192) {
+        if (PROBE(p.debug_mode, 8192)) {
           mbar_arrive(full_bar + s);
         } else {
           mbar_expect_tx(full_bar + s, p.np * 128);
@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
           }
           const int kk = pn * KR + k;
           const int cl = (a * 128 + c16 * 16) / EB;     // column inside the 128-column panel
-          const bool ok = kk < p.n_loc && j0 + cl < p.N && !(p.debug_mode & 8192);
+          const bool ok = kk < p.n_loc && j0 + cl < p.N && !PROBE(p.debug_mode, 8192);
           const uint32_t rowp = ok ? (rw_s[kk] & 0x3FFFFFFFu) : 0u;
           // panel layout [column tile][m][128]: the rows of one tile are 128 * EB bytes apart
           cp_async16(ws + dst_off, Wb + ((uint64_t)rowp * 128 + (ok ? cl : 0)) * EB, ok ? 16u : 0u);
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     const int jl = 32 * q4 + lane;
     const int j = j0 + jl;
     const bool jok = j < p.N;
-    const bool do_store = jok && !(p.debug_mode & 1024);           // bit 10: no stores (timing probe)
+    const bool do_store = jok && !PROBE(p.debug_mode, 1024);           // bit 10: no stores (timing probe)
     const bool has_shadow = p.Wnext != nullptr;
     const uint32_t tile_m = (uint32_t)(blockIdx.x * p.m);
     constexpr uint32_t ROWB = 128 * sizeof(S);          // bytes of one row of a panel
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     constexpr int RSTEP = 32 / PPR;                     // rows covered by the 32 lanes: 4 / 2
     const int t_lane = lane / PPR;
     const int pc = lane % PPR;
-    const bool colok = j0 + 32 * q4 + pc * (16 / (int)sizeof(S)) < p.N && !(p.debug_mode & 2048);   // bit 11: no epilogue loads (probe)
+    const bool colok = j0 + 32 * q4 + pc * (16 / (int)sizeof(S)) < p.N && !PROBE(p.debug_mode, 2048);   // bit 11: no epilogue loads (probe)
     const uint32_t col_bytes = (uint32_t)(32 * q4 * (int)sizeof(S) + pc * 16);
     const uint64_t srcRX = (uint64_t)__cvta_generic_to_global(p.RX) + col_bytes;
     const uint64_t srcRY = (uint64_t)__cvta_generic_to_global(p.RY) + col_bytes;
@@ -247,8 +247,8 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     const uint32_t g_rowb = g_rm ? (uint32_t)p.N * (uint32_t)sizeof(S) : ROWB;
     const uint32_t g_sub = g_rm ? tile_m : 0u;
     const uint64_t srcG = (uint64_t)__cvta_generic_to_global(has_g ? p.G : p.RX) + col_bytes + (g_rm ? (uint64_t)j0 * sizeof(S) : (uint64_t)0);
-    const bool g_ok = has_g && !(p.debug_mode & 4096);              // bit 12: no R_Y / G loads (timing probe)
-    const bool ry_ok = !(p.debug_mode & 4096);
+    const bool g_ok = has_g && !PROBE(p.debug_mode, 4096);              // bit 12: no R_Y / G loads (timing probe)
+    const bool ry_ok = !PROBE(p.debug_mode, 4096);
     const uint32_t ring_lane = smem_u32(ring) + (uint32_t)(t_lane * SEG + pc * 16);
     const uint32_t *rw_lane = rw_s + sub * RW + t_lane;
     const int a_lane = sub * RW + t_lane;
@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
     };
     mbar_wait(accum_bar, 0);     // every MMA done: TMEM complete, operand stages free for the rings
     tc_fence_after();
-    if (!(p.debug_mode & 4)) {
+    if (!PROBE(p.debug_mode, 4)) {
 #pragma unroll
       for (int c = 0; c < FE_DEPTH - 1; ++c) issue_chunk(c);
       // accumulator columns of chunk c + 1 are requested while chunk c is processed

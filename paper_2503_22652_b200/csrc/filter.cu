@@ -1,5 +1,6 @@
 // rchfsi_filter / rchfsi_filter_host / rchfsi_solve: host control flow of Algorithm 2
 // (PAPER.md:78-86), Algorithm 3 and Algorithm 1.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include "common.cuh"
@@ -44,12 +45,13 @@ Plan make_plan(const rchfsi_ctx *h) {
   // before its epilogue starts: the new shadow may overwrite the old one, one buffer instead of two
   // (14.8 GB instead of 29.6 GB of BF16 shadows at config 5).  The dense step cannot: its row tiles read all rows.
   // RCHFSI_FE_SHADOW_PAIR=1 keeps the two-buffer scheme (the tests compare the two bit for bit).
-  p.shadow_inplace = p.shadow && p.fused == 3 && !getenv("RCHFSI_FE_SHADOW_PAIR");
+  p.shadow_inplace = p.shadow && p.fused == 3 && !h->knobs.fe_shadow_pair;
   return p;
 }
 
 rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t degree, bool need_gs) {
-  const size_t el = (size_t)h->m * (pl.panel ? (size_t)cdiv(h->N, 128) * 128 : (size_t)h->N);
+  // sized for the block width of rchfsi_create (N_cap), whatever the active width of this call
+  const size_t el = (size_t)h->m * (pl.panel ? (size_t)cdiv(h->N_cap, 128) * 128 : (size_t)h->N_cap);
   if (!h->RX) RCHFSI_TRY(dev_alloc(h, &h->RX, el * prec_bytes(pl.store)));
   if (!h->RY) RCHFSI_TRY(dev_alloc(h, &h->RY, el * prec_bytes(pl.store)));
   if (pl.shadow) {
@@ -60,10 +62,10 @@ rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t deg
   if (pl.fused == 0 && !h->T) RCHFSI_TRY(dev_alloc(h, &h->T, el * prec_bytes(pl.tprec)));
   if (need_gs && !h->Gs) RCHFSI_TRY(dev_alloc(h, &h->Gs, el * prec_bytes(pl.store)));
   if (!h->lam_table || h->lam_table_p < degree) {
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->lam_table, sizeof(double) * (size_t)(degree + 1) * h->N));
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->lam_table, sizeof(double) * (size_t)(degree + 1) * h->N_cap));
     h->lam_table_p = degree;
   }
-  if (!h->colnorm) RCHFSI_TRY(dev_alloc(h, (void **)&h->colnorm, sizeof(double) * 2 * h->N));
+  if (!h->colnorm) RCHFSI_TRY(dev_alloc(h, (void **)&h->colnorm, sizeof(double) * 2 * h->N_cap));
   return RCHFSI_OK;
 }
 
@@ -139,8 +141,9 @@ static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, con
   if (!chfsi) {
     // G = A X - B X Lambda with the exact operators (reading S5) when the caller has none
     if (!G) {
-      if (!h->Gtmp) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gtmp, el * 8));
-      if (!h->rr1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr1, el * 8));
+      const size_t el_cap = (size_t)m * h->N_cap;
+      if (!h->Gtmp) RCHFSI_TRY(dev_alloc(h, (void **)&h->Gtmp, el_cap * 8));
+      if (!h->rr1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rr1, el_cap * 8));
       RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, X, h->rr1, N));
       const double *BX = X;
       if (h->B.present) {
@@ -215,43 +218,95 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   return filter_impl(h, method, X, ritz, G, h->opt.g_input_f32 != 0, degree, lam_min, lam_T, lam_max);
 }
 
+// Column-chunked host pipeline.  The columns of the block are independent through the whole filter (Alg. 3 touches
+// column j only through eps_j and Lambda_k[j]), so the block is cut into column chunks and chunk
+// i+1 is uploaded while chunk i is filtered and chunk i-1 is downloaded: three streams, three staging sets.
+static int32_t host_chunk_width(const rchfsi_ctx *h) {
+  const int32_t N = h->N_cap;
+  const double blk = 8.0 * (double)h->m * N;
+  if (blk < 256e6 || N < 512) return N;               // small blocks: one chunk (the X upload still overlaps the steps)
+  int32_t w = (int32_t)cdiv(cdiv(N, 6), 128) * 128;   // about six chunks, whole 128-column tiles
+  return std::min(w, N);
+}
+
 rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host, const double *ritz_host,
                                  const double *G_host, int32_t degree, double lam_min, double lam_T,
                                  double lam_max) {
   if (!h) return RCHFSI_EINVAL;
   if (!X_host || (method == RCHFSI_METHOD_RCHFSI && !ritz_host)) { h->err = "rchfsi_filter_host: null argument"; return RCHFSI_EINVAL; }
-  const size_t blk = sizeof(double) * (size_t)h->m * h->N;
+  if (h->N != h->N_cap) { h->err = "rchfsi_filter_host: handle is inside another call"; return RCHFSI_EINVAL; }
+  const int64_t m = h->m;
+  const int32_t N = h->N_cap;
+  const bool gf32 = h->opt.g_input_f32 != 0;
+  const size_t gb = gf32 ? 4 : 8;                       // bytes per element of G_host (FP32 with g_input_f32)
   cudaStream_t st = h->stream;
-  if (!h->hX) RCHFSI_TRY(dev_alloc(h, (void **)&h->hX, blk));
-  if (!h->hritz) RCHFSI_TRY(dev_alloc(h, (void **)&h->hritz, sizeof(double) * h->N));
-  if (G_host && !h->hG) RCHFSI_TRY(dev_alloc(h, (void **)&h->hG, blk));
-  // Alg. 3 with the residual block given reads X only in its last line: its copy goes on a second
-  // stream and overlaps the p-1 recurrence steps; G and the Ritz values are needed first and go ahead of the kernels
-  h->x_pending = false;
-  const bool overlap_x = (method == RCHFSI_METHOD_RCHFSI) && G_host != nullptr;
-  if (overlap_x) {
-    if (!h->copy_stream) RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
-    if (!h->ev_x) RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_x, cudaEventDisableTiming));
-    if (G_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hG, G_host, blk, cudaMemcpyHostToDevice, st));
-    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * h->N, cudaMemcpyHostToDevice, st));
-    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hX, X_host, blk, cudaMemcpyHostToDevice, h->copy_stream));
-    RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_x, h->copy_stream));
-    h->x_pending = true;
-  } else {
-    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hX, X_host, blk, cudaMemcpyHostToDevice, st));
-    if (ritz_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * h->N, cudaMemcpyHostToDevice, st));
-    if (G_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hG, G_host, blk, cudaMemcpyHostToDevice, st));
+  const int32_t w = host_chunk_width(h);
+  const int nchunks = (int)cdiv(N, w);
+  const int nsets = std::min<int>(rchfsi_ctx::HOST_SETS, nchunks);
+  if (h->host_chunk != w) {
+    if (h->host_chunk != 0) { h->err = "rchfsi_filter_host: staging width changed"; return RCHFSI_EINVAL; }
+    for (int i = 0; i < nsets; ++i) {
+      RCHFSI_TRY(dev_alloc(h, (void **)&h->hX[i], sizeof(double) * (size_t)m * w));
+      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_g[i], cudaEventDisableTiming));
+      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_xin[i], cudaEventDisableTiming));
+      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_free[i], cudaEventDisableTiming));
+    }
+    RCHFSI_TRY(dev_alloc(h, (void **)&h->hritz, sizeof(double) * N));
+    RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
+    RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
+    h->host_chunk = w;
   }
-  rchfsi_status fst = rchfsi_filter(h, method, h->hX, ritz_host ? h->hritz : nullptr, G_host ? h->hG : nullptr, degree,
-                                    lam_min, lam_T, lam_max);
-  if (h->x_pending) {   // the filter returned before its last line (invalid arguments): do not leave the copy in flight
-    h->x_pending = false;
-    cudaStreamSynchronize(h->copy_stream);
+  if (G_host)
+    for (int i = 0; i < nsets; ++i)
+      if (!h->hG[i]) RCHFSI_TRY(dev_alloc(h, &h->hG[i], gb * (size_t)m * w));
+  if (ritz_host) RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(h->hritz, ritz_host, sizeof(double) * N, cudaMemcpyHostToDevice, st));
+  // everything enqueued earlier on the main stream (previous calls reading the staging sets) is ordered first
+  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_free[0], st));
+  RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(h->in_stream, h->ev_free[0], 0));
+  RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(h->out_stream, h->ev_free[0], 0));
+  rchfsi_status result = RCHFSI_OK;
+  for (int c = 0; c < nchunks && result == RCHFSI_OK; ++c) {
+    const int b = c % nsets;
+    const int32_t j0 = c * w, wc = std::min<int32_t>(w, N - j0);
+    // ---- upload (in_stream): G first, it is what the recurrence needs; X is read only by the last line
+    if (c >= nsets) RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(h->in_stream, h->ev_free[b], 0));
+    if (G_host)
+      RCHFSI_CUDA_CHECK(h, cudaMemcpy2DAsync(h->hG[b], gb * wc, reinterpret_cast<const char *>(G_host) + gb * j0, gb * N,
+                                             gb * wc, (size_t)m, cudaMemcpyHostToDevice, h->in_stream));
+    RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_g[b], h->in_stream));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpy2DAsync(h->hX[b], sizeof(double) * wc, X_host + j0, sizeof(double) * N,
+                                           sizeof(double) * wc, (size_t)m, cudaMemcpyHostToDevice, h->in_stream));
+    RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_xin[b], h->in_stream));
+    // ---- filter the chunk (main stream) as a block of width wc
+    RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(st, h->ev_g[b], 0));
+    const bool late_x = (method == RCHFSI_METHOD_RCHFSI) && G_host != nullptr;
+    if (late_x) {
+      h->ev_x = h->ev_xin[b];
+      h->x_pending = true;
+    } else {
+      RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(st, h->ev_xin[b], 0));
+    }
+    h->N = wc;
+    result = filter_impl(h, method, h->hX[b], ritz_host ? h->hritz + j0 : nullptr, G_host ? h->hG[b] : nullptr, gf32,
+                         degree, lam_min, lam_T, lam_max);
+    h->N = N;
+    if (h->x_pending) {   // the filter returned before its last line (invalid arguments)
+      h->x_pending = false;
+      cudaStreamSynchronize(h->in_stream);
+    }
+    if (result != RCHFSI_OK) break;
+    RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_done[b], st));
+    // ---- download (out_stream)
+    RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(h->out_stream, h->ev_done[b], 0));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpy2DAsync(X_host + j0, sizeof(double) * N, h->hX[b], sizeof(double) * wc,
+                                           sizeof(double) * wc, (size_t)m, cudaMemcpyDeviceToHost, h->out_stream));
+    RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_free[b], h->out_stream));
   }
-  RCHFSI_TRY(fst);
-  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(X_host, h->hX, blk, cudaMemcpyDeviceToHost, st));
+  cudaStreamSynchronize(h->in_stream);
+  cudaStreamSynchronize(h->out_stream);
   RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(st));
-  return RCHFSI_OK;
+  return result;
 }
 
 rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n_wanted, int32_t degree,

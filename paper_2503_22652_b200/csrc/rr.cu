@@ -30,7 +30,7 @@ struct PhaseTimer {
   rchfsi_ctx *h;
   bool on;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
-  explicit PhaseTimer(rchfsi_ctx *hh) : h(hh), on(getenv("RCHFSI_RR_TIMING") != nullptr) {
+  explicit PhaseTimer(rchfsi_ctx *hh) : h(hh), on(hh->knobs.rr_timing) {
     if (on) {
       cudaEventCreate(&e0);
       cudaEventCreate(&e1);
@@ -207,7 +207,7 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
 // Chunked variant: no full-size temporary.  Extra device memory: two [m][cw] FP64 chunks and one [rp][N]
 // FP64 row panel (about 6 GB + 3 GB at config 5 instead of 3 x 58.5 GB).
 bool rr_wants_chunked(rchfsi_ctx *h) {
-  if (const char *e = getenv("RCHFSI_RR_CHUNKED")) return atoi(e) != 0;      // test / tuning knob
+  if (h->knobs.rr_chunked >= 0) return h->knobs.rr_chunked != 0;               // test / tuning knob
   if (h->rrc1) return true;                                                    // decided earlier for this handle
   if (h->rr1) return false;                                                    // full workspace already there
   size_t free_b = 0, total_b = 0;

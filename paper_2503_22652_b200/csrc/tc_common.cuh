@@ -1,4 +1,4 @@
-// sm_100a building blocks for the tensor-core paths: mbarrier, TMA (tiled and tile::gather4),
+// sm_100a building blocks for the tensor-core paths: mbarrier, TMA (tiled, multicast),
 // tcgen05 (alloc / mma / commit / ld) wrappers in inline PTX, and the shared-memory / instruction
 // descriptors for the canonical SWIZZLE_128B layouts.
 #pragma once
@@ -18,7 +18,6 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
 __device__ __forceinline__ void fence_barrier_init() {
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
@@ -94,15 +93,6 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
   asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
   return r;
 }
-// four rows r0..r3 of a 2D tensor, box width columns starting at x, landing as 4 consecutive rows
-__device__ __forceinline__ void tma_gather4(void *smem_dst, const CUtensorMap *m, uint64_t *bar, int32_t x, int32_t r0,
-                                            int32_t r1, int32_t r2, int32_t r3) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cta.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, "
-      "%7}], [%2];" ::"r"(smem_u32(smem_dst)),
-      "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar)), "r"(x), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
-      : "memory");
-}
 
 // ------------------------------------------------------------------- cp.async (LDGSTS)
 // 16-byte global -> shared copy; src_bytes = 0 zero-fills the destination without reading
@@ -122,10 +112,6 @@ __device__ __forceinline__ void st_global(uint64_t addr, double v) { asm volatil
 __device__ __forceinline__ void st_global_u32(uint64_t addr, uint32_t v) { asm volatile("st.global.u32 [%0], %1;" ::"l"(addr), "r"(v) : "memory"); }
 __device__ __forceinline__ void st_global_u16(uint64_t addr, uint16_t v) { asm volatile("st.global.u16 [%0], %1;" ::"l"(addr), "h"(v) : "memory"); }
 __device__ __forceinline__ void cp_async16_sa(uint32_t smem_dst, uint64_t gsrc, uint32_t src_bytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
-}
-// the same with the destination given as a 32-bit shared-window address
-__device__ __forceinline__ void cp_async16_s(uint32_t smem_dst, const void *gsrc, uint32_t src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
 }
 // the mbarrier receives one arrival from this thread when all its earlier cp.async have landed
@@ -192,15 +178,6 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
       : "r"(taddr)
       : "memory");
 }
-__device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t (&r)[16]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-      : "r"(taddr)
-      : "memory");
-}
 __device__ __forceinline__ void tmem_ld_32x8(uint32_t taddr, uint32_t (&r)[8]) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
@@ -250,7 +227,7 @@ bool make_tmap_2d(CUtensorMap *out, const void *base, int elem_bytes, bool bf16,
 
 struct rchfsi_ctx;
 namespace rchfsi {
-// cached variant: returns nullptr on failure
-const CUtensorMap *get_tmap_2d(rchfsi_ctx *h, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
-                               uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32 = 0);
+// cached variant: the descriptor is COPIED into *out (the cache may reallocate or evict); false on failure
+bool get_tmap_2d(rchfsi_ctx *h, CUtensorMap *out, const void *base, int elem_bytes, bool bf16, uint64_t rows, uint64_t cols,
+                 uint64_t pitch_bytes, uint32_t box_cols, uint32_t box_rows, int atom32 = 0);
 }  // namespace rchfsi

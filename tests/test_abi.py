@@ -36,7 +36,7 @@ def test_default_options_and_struct_layout():
     opt.apply_prec = 99
     lib.rchfsi_default_options(C.byref(opt))
     assert (opt.apply_prec, opt.store_prec, opt.normalize_columns_before_rr) == (P.FP64, P.FP64, 1)
-    assert (opt.adaptive_bounds, opt.noise_eps, opt.noise_seed, opt.use_cuda_graph) == (0, 0.0, 0, 0)
+    assert (opt.adaptive_bounds, opt.noise_eps, opt.noise_seed, opt.g_input_f32) == (0, 0.0, 0, 0)
     assert C.sizeof(P.RchfsiOptions) == 40
     assert C.sizeof(P.RchfsiOperator) == 104
 

@@ -308,7 +308,7 @@ def test_dense_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_
 @pytest.mark.parametrize("apply_prec,tol", [("tf32", 6e-3), ("bf16", 3e-2)])
 @pytest.mark.parametrize("nc,q,N,p", [(2, 6, 136, 3), (3, 3, 16, 4), (3, 2, 264, 3)])
 def test_fe_tensor_core_step_is_the_oracle_step_up_to_operand_rounding(apply_prec, tol, nc, q, N, p):
-    """FE tcgen05 path (TMA gather4 prologue, coloured atomic-free scatter fused with the update):
+    """FE tcgen05 path (cp.async gather into the swizzled UMMA layout, coloured atomic-free scatter fused with the update):
     the residual part of the filtered block equals the oracle's up to operand rounding (tolerances
     as for the dense kernel).  q=6: 343 nodes per cell, two 176-wide accumulator halves, ragged K
     tail; q=2,3: single accumulator; N=136/264: a ragged second/third 128-column tile."""
