@@ -75,6 +75,8 @@ static Knobs read_knobs() {
   k.rr_fe_simt = getenv("RCHFSI_RR_FE_SIMT") != nullptr;
   k.rr_timing = getenv("RCHFSI_RR_TIMING") != nullptr;
   k.rr_split = geti("RCHFSI_RR_SPLIT", -1);
+  k.host_chunk = geti("RCHFSI_HOST_CHUNK", 0);
+  k.csr_variant = geti("RCHFSI_CSR_VARIANT", 0);
 #ifdef RCHFSI_PROBES
   k.tc_debug = geti("RCHFSI_TC_DEBUG", 0);
 #endif
@@ -117,6 +119,11 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const 
   h->opt = o;
   h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->knobs = read_knobs();
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || h->num_sms <= 0) h->num_sms = 148;
+  }
   for (const rchfsi_operator *op : {A, B}) {
     if (op && op->kind == RCHFSI_OP_FE) {
       double asym = 0.0;

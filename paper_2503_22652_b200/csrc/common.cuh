@@ -58,6 +58,8 @@ struct Knobs {
   bool rr_fe_simt = false;       // RCHFSI_RR_FE_SIMT: FE applies of the Rayleigh-Ritz through the hand-written FP64 kernel
   bool rr_timing = false;        // RCHFSI_RR_TIMING: print phase times of the Rayleigh-Ritz to stderr
   int rr_split = -1;             // RCHFSI_RR_SPLIT: Gram / rotation products on the tensor pipe (split operands), -1 = automatic
+  int csr_variant = 0;           // RCHFSI_CSR_VARIANT: tuning sweep of the fused CSR step (0 = round-1 kernel)
+  int host_chunk = 0;            // RCHFSI_HOST_CHUNK: column-chunk width of rchfsi_filter_host (multiple of 128), 0 = automatic
   int tc_debug = 0;              // RCHFSI_TC_DEBUG (only in -DRCHFSI_PROBES builds)
 };
 
@@ -88,6 +90,7 @@ struct rchfsi_ctx {
   cusolverDnHandle_t cusolver = nullptr;
   std::string err;
   int64_t launches = 0;
+  int num_sms = 0;                       // multiprocessors of the current device (persistent-kernel grids)
 
   // filter workspace (storage precision), lazily allocated
   void *RX = nullptr, *RY = nullptr;      // [m][N] store_prec

@@ -359,4 +359,5 @@ __global__ void __launch_bounds__(FE_THREADS, 1) fe_tc_kernel(const __grid_const
 }  // namespace
 }  // namespace rchfsi
 
+#include "fe_pipe.inc"
 #include "fe_tc_host.inc"

@@ -223,6 +223,7 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
 // i+1 is uploaded while chunk i is filtered and chunk i-1 is downloaded: three streams, three staging sets.
 static int32_t host_chunk_width(const rchfsi_ctx *h) {
   const int32_t N = h->N_cap;
+  if (h->knobs.host_chunk >= 128) return std::min<int32_t>((int32_t)cdiv(h->knobs.host_chunk, 128) * 128, N);   // test knob
   const double blk = 8.0 * (double)h->m * N;
   if (blk < 256e6 || N < 512) return N;               // small blocks: one chunk (the X upload still overlaps the steps)
   int32_t w = (int32_t)cdiv(cdiv(N, 6), 128) * 128;   // about six chunks, whole 128-column tiles

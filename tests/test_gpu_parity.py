@@ -239,6 +239,102 @@ def test_filter_host_entry_point_equals_device_entry_point():
     solver.close()
 
 
+@pytest.mark.parametrize("kind,apply_prec,store", [("fe", "bf16", "fp32"), ("fe", "tf32", "fp64"), ("csr", "fp32", "fp64"),
+                                                   ("dense", "fp64", "fp64")])
+def test_filter_host_column_chunks_equal_the_device_entry_point_bitwise(monkeypatch, kind, apply_prec, store):
+    """rchfsi_filter_host cuts the block into column chunks (three streams: upload chunk i+1, filter chunk i, download
+    chunk i-1); the columns are independent through the whole filter, so the result must be
+    bit for bit the device entry point's.  RCHFSI_HOST_CHUNK=128 forces three chunks (128 + 128 + 8 columns)."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_HOST_CHUNK", "128")
+    N, p = 264, 6
+    if kind == "fe":
+        prob = workloads.fe_problem(2, q=3, seed=51)
+        lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    elif kind == "csr":
+        prob = workloads.config3_sparse_laplacian(n=9, n_wanted=10, block=N, degree=p, seed=6)
+        lam_max = 12.0
+    else:
+        prob = small_dense_generalized(300, seed=9)
+        lam_max = 16.0
+    solver, _, X, ritz, G = _setup(prob, N, 23, apply_prec=apply_prec, store_prec=store)
+    b = (ritz[0] - 1.0, ritz[-1] + 1.0, lam_max)
+    for method in (P.METHOD_RCHFSI, P.METHOD_CHFSI):
+        Xd = torch.as_tensor(X).cuda()
+        solver.filter(method, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *b)
+        Xh = torch.as_tensor(X.copy()).pin_memory()
+        solver.filter_host(method, Xh, ritz, G, p, *b)
+        np.testing.assert_array_equal(Xh.numpy(), Xd.cpu().numpy())
+    with pytest.raises(TypeError):      # the binding validates host arrays (dtype / shape / contiguity)
+        solver.filter_host(P.METHOD_RCHFSI, X.astype(np.float32), ritz, G, p, *b)
+    solver.close()
+
+
+def test_filter_host_takes_an_fp32_residual_block_with_g_input_f32():
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = workloads.fe_problem(2, q=3, seed=52)
+    lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    N, p = 136, 5
+    solver, _, X, ritz, G = _setup(prob, N, 24, apply_prec="bf16", store_prec="fp32", g_input_f32=True)
+    b = (ritz[0] - 1.0, ritz[-1] + 1.0, lam_max)
+    G32 = G.astype(np.float32)
+    Xd = torch.as_tensor(X).cuda()
+    solver.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G32).cuda(), p, *b)
+    Xh = X.copy()
+    solver.filter_host(P.METHOD_RCHFSI, Xh, ritz, G32, p, *b)
+    np.testing.assert_array_equal(Xh, Xd.cpu().numpy())
+    with pytest.raises(TypeError):      # an FP64 host G would be misread as FP32
+        solver.filter_host(P.METHOD_RCHFSI, Xh, ritz, G, p, *b)
+    solver.close()
+
+
+def test_fe_mesh_with_a_row_no_cell_touches_is_rejected_at_create():
+    """A global row referenced by no cell has no first toucher in the coloured scatter (it would keep stale data):
+    rchfsi_create returns EINVAL instead."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = dict(workloads.fe_problem(2, q=2, seed=3))
+    prob["m"] = prob["m"] + 1                      # one extra, uncovered row
+    prob["dinv"] = np.concatenate((prob["dinv"], [1.0]))
+    As, Bs, dinv = P.upload_problem(prob)
+    with pytest.raises(P.RchfsiError) as ei:
+        P.Rchfsi(As, Bs, dinv, block_N=8)
+    assert ei.value.status == P.EINVAL and "belongs to no cell" in str(ei.value)
+
+
+def test_operator_changed_drops_the_reduced_precision_copies():
+    """The filter keeps a reduced-precision copy of A with D^-1 folded in; after the caller rewrites A in place,
+    rchfsi_operator_changed makes the next filter see the new operator."""
+    torch = _torch()
+    import paper_2503_22652_b200 as P
+    prob = small_dense_generalized(256, seed=12)
+    N, p = 16, 4
+    A, B, Dinv = oracle_ops(prob)
+    X0 = np.random.default_rng(1).standard_normal((prob["m"], N))
+    ritz, X, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, X0)
+    G = orc.residual_block(AX, BX, ritz)
+    As, Bs, dinv = P.upload_problem(prob)
+    s = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec="tf32")
+    b = (ritz[0] - 1.0, ritz[-1] + 1.0, 16.0)
+    rd, Gd = torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda()
+    X1 = torch.as_tensor(X).cuda()
+    s.filter(P.METHOD_RCHFSI, X1, rd, Gd, p, *b)
+    As["A"].mul_(0.5)                               # the caller's operator evolves in place
+    X2 = torch.as_tensor(X).cuda()
+    s.filter(P.METHOD_RCHFSI, X2, rd, Gd, p, *b)    # stale copy: same result as before
+    assert torch.equal(X1, X2)
+    s.operator_changed()
+    X3 = torch.as_tensor(X).cuda()
+    s.filter(P.METHOD_RCHFSI, X3, rd, Gd, p, *b)
+    Yo = orc.filter_rchfsi(orc.DenseOperator(0.5 * prob["A"]).apply, Dinv.apply, X, ritz, G, p, *b)
+    XL = X * orc.lambda_recurrence(ritz, p, *b)[p][None, :]
+    assert rel_fro(X3.cpu().numpy() - XL, Yo - XL) < 6e-3
+    assert not torch.equal(X1, X3)
+    s.close()
+
+
 def test_filter_rejects_bad_arguments_without_touching_X():
     torch = _torch()
     import paper_2503_22652_b200 as P
