@@ -23,9 +23,12 @@
  *    void*, NULL = the legacy default stream).  rchfsi_filter and rchfsi_rayleigh_ritz are
  *    asynchronous with respect to the host; rchfsi_solve and the *_host entry points
  *    synchronise the stream before returning.
- *  - The library allocates its own device workspace (recurrence blocks, low-precision
- *    operator copies, Rayleigh-Ritz temporaries) with cudaMalloc, lazily, and frees it in
- *    rchfsi_destroy.  rchfsi_workspace_bytes reports the worst case up front.
+ *  - The library never allocates device memory.  Its workspace (recurrence blocks, reduced-
+ *    precision operator copies, Rayleigh-Ritz temporaries, staging of the host entry point)
+ *    is carved from caller-provided device buffers (rchfsi_add_workspace; e.g. torch tensors).
+ *    rchfsi_workspace_bytes plans the size of a single sufficient buffer up front; a call that
+ *    runs out returns RCHFSI_ENOMEM before it has changed any caller block, reports the missing
+ *    bytes (rchfsi_workspace_shortfall) and may simply be repeated after adding a segment.
  *  - There is no CPU fallback: without a CUDA device every compute entry point returns
  *    RCHFSI_ECUDA.
  */
@@ -44,7 +47,7 @@ typedef struct rchfsi_ctx *rchfsi_handle;
 typedef enum {
   RCHFSI_OK = 0,
   RCHFSI_EINVAL = 1,         /* bad argument; outputs untouched */
-  RCHFSI_ENOMEM = 2,         /* cudaMalloc / malloc failed */
+  RCHFSI_ENOMEM = 2,         /* the workspace is exhausted (rchfsi_workspace_shortfall), or malloc failed */
   RCHFSI_ECUDA = 3,          /* CUDA / cuBLAS / cuSOLVER runtime error, or no device */
   RCHFSI_ENOTCONVERGED = 4,  /* rchfsi_solve hit max_iter; outputs hold the last iterate */
   RCHFSI_EBREAKDOWN = 5      /* Rayleigh-Ritz Gram matrix Y^T B Y not numerically SPD */
@@ -106,6 +109,8 @@ typedef struct {
                                  T_j += eps ||T_j|| g_j/||g_j|| inside the filter only
                                  (BASELINE.json configs[0]; reading S11) */
   uint64_t noise_seed;
+  int32_t allow_high_degree;  /* the filter refuses degree >= 100 with a reduced-precision apply (the paper finds p = 100,
+                                 120 unstable in FP32 / TF32, PAPER.md:347-359 and footnote 5) unless this is set */
   int32_t g_input_f32;        /* nonzero: the G argument of rchfsi_filter points to FP32 values [m][N] (an FP64
                                  residual block does not fit at config 5, SURVEY 8(d) memory plan); needs
                                  store_prec FP32; G is then read in place, no copy is made */
@@ -140,10 +145,25 @@ rchfsi_status rchfsi_operator_changed(rchfsi_handle h);
  * message of the last failed rchfsi_create in this thread. */
 const char *rchfsi_last_error(rchfsi_handle h);
 
-/* Worst-case device bytes the handle will allocate for the given problem (recurrence
- * blocks + low-precision operator copy + Rayleigh-Ritz temporaries). */
-size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B,
-                              int32_t block_N, const rchfsi_options *opt);
+/* Workspace ("the caller (torch) allocates the workspace").
+ * rchfsi_workspace_bytes: bytes of ONE device buffer that is sufficient for the entry points named in `uses`
+ *   (bit-or of rchfsi_use) with filter degrees up to max_degree; computed from the descriptors alone (no device
+ *   needed).  It enumerates the same buffers as the allocation sites; for the memory-light Rayleigh-Ritz of
+ *   rchfsi_solve (chosen when three more FP64 blocks do not fit on the device) less is used.
+ * rchfsi_add_workspace: hand `bytes` of device memory (borrowed until rchfsi_destroy; any alignment) to the handle.
+ *   May be called several times; buffers never span segments.
+ * rchfsi_workspace_shortfall: after an RCHFSI_ENOMEM, the size of a segment that lets the failed allocation
+ *   succeed (0 otherwise).  rchfsi_workspace_used: bytes handed out so far. */
+typedef enum {
+  RCHFSI_USE_FILTER = 1, RCHFSI_USE_RAYLEIGH_RITZ = 2, RCHFSI_USE_SOLVE = 4, RCHFSI_USE_FILTER_HOST = 8,
+  RCHFSI_USE_BOUNDS = 16,
+  RCHFSI_USE_FILTER_NULL_G = 32   /* rchfsi_filter will be called with G == NULL (two more FP64 blocks) */
+} rchfsi_use;
+size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B, int32_t block_N,
+                              const rchfsi_options *opt, int32_t uses, int32_t max_degree);
+rchfsi_status rchfsi_add_workspace(rchfsi_handle h, void *device_buffer, size_t bytes);
+size_t rchfsi_workspace_shortfall(rchfsi_handle h);
+size_t rchfsi_workspace_used(rchfsi_handle h);
 
 /* The Chebyshev filter (the hot path).
  *  method RCHFSI (Algorithm 3):
@@ -159,7 +179,8 @@ size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B
  *  ritz   device [N] FP64: diagonal of Lambda^(i) (RCHFSI only; ignored for CHFSI).
  *  G      device [m][N] FP64: A X - B X Lambda computed with the exact
  *         operators; NULL => computed here in FP64 from A, B, X, ritz (RCHFSI only).
- *  degree p >= 1; lam_min < lam_T < lam_max (a_low <= lambda_1, [a,b] = [lam_T, lam_max]).
+ *  degree p >= 1 (p >= 100 with a reduced-precision apply needs allow_high_degree);
+ *  lam_min < lam_T < lam_max (a_low <= lambda_1, [a,b] = [lam_T, lam_max]).
  * Asynchronous.  Errors: EINVAL (bad handle / pointers / degree / bounds), ECUDA, ENOMEM. */
 rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const double *ritz,
                             const double *G, int32_t degree, double lam_min, double lam_T,
@@ -194,6 +215,31 @@ rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n
                            int32_t degree, double lam_min, double lam_T, double lam_max,
                            double tol, int32_t max_iter, double *evals_out,
                            double *resnorm_out, int32_t *iters_out, double *history_out);
+
+/* Estimates of the upper spectral bound lam_max the filter is parameterised by ("parameterised by
+ * estimates lam_min, lam_max, lam_T").  The recurrence applies D^-1 A (eq. (7) at PAPER.md:170, Algorithm 3 at 263),
+ * so lam_max must bound lam(D^-1 A); it should also bound lam(B^-1 A).  All computed on the device, FP64:
+ *   lanczos_*        k-step Lanczos on D^-1/2 A D^-1/2 from a Gaussian start vector drawn from `seed` by the
+ *                    counter-based generator of the noise hook: extreme Ritz values theta_min / theta_max (inside the
+ *                    spectrum) and lanczos_max = theta_max + beta_k |s_k| (Ritz value + its residual norm);
+ *   gershgorin_max   ||D^-1 A||_inf = max_i d_i sum_j |a_ij|: rigorous for lam(D^-1 A), usually loose;
+ *   fe_cellwise_max  A and B FE operators on one mesh: max_c lam_max(A_c, B_c) >= lam_max(A, B) over every
+ *                    fe_cell_stride-th cell (each cell pencil by cuSOLVER); rigorous for stride 1, NaN when it does
+ *                    not apply or fe_cell_stride == 0;
+ *   lam_max          recommended value: lanczos_max + 1 %, capped by gershgorin_max, raised to fe_cellwise_max
+ *                    (+ 2 % when only a sample of the cells was examined).
+ * Synchronises the stream.  Errors: EINVAL (steps outside [2, 512]), ECUDA, ENOMEM, EBREAKDOWN. */
+typedef struct {
+  double lam_max;
+  double lanczos_max;
+  double lanczos_theta_max;
+  double lanczos_theta_min;
+  double gershgorin_max;
+  double fe_cellwise_max;
+  int32_t lanczos_steps;      /* steps actually taken (fewer on an invariant subspace) */
+} rchfsi_bounds;
+rchfsi_status rchfsi_estimate_bounds(rchfsi_handle h, int32_t lanczos_steps, int32_t fe_cell_stride, uint64_t seed,
+                                     rchfsi_bounds *out);
 
 /* Exact FP64 operator apply, exposed for tests and residual certification:
  * which = 0: out = A V, which = 1: out = B V (B = I copies).  V, out device [m][N]. */

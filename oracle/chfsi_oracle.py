@@ -17,6 +17,10 @@ so that it can be checked against PAPER.md by eye:
   residual_norms      r_j = ||A x_j - eps_j B x_j||_2
   solve               Algorithm 1 (do-while reading S1)
   tan_max_angle       Definition 2.1
+  lanczos_upper_bound estimate of lam_max ("estimates lam_min, lam_max, lam_T"):
+                      k-step Lanczos on D^-1/2 A D^-1/2, theta_max + its residual beta_k |s_k|
+  gershgorin_upper    max_i d_i sum_j |a_ij| >= lam_max(D^-1 A)   (rigorous)
+  fe_cellwise_upper   max_c lam_max(A_c, B_c) >= lam_max(A, B)     (rigorous; SURVEY reading S7)
 
 Operators are objects with ``apply(V) -> A V`` on an [m][N] float64 block:
 DenseOperator (a matmul), CsrOperator (library SpMM of the CSR triplet),
@@ -290,6 +294,69 @@ def solve(A_exact, B_exact, A_filter, Dinv, X0, n_wanted, p, lam_min, lam_T, lam
         if early_stop and history[-1] < tol:
             break
     return dict(evals=ritz, X=X, resnorm=r, iters=it, history=history)
+
+
+# --------------------------------------------------------------------------- spectral bounds
+def lanczos_upper_bound(apply_A, dinv, v0, k):
+    """The filter is "parameterised by estimates lam_min, lam_max, lam_T" and
+    lam_max must bound lam(D^-1 A) (the operator the recurrence applies, eq. (7) / Alg. 3).
+    k-step Lanczos (no reorthogonalisation) on the symmetric S = D^-1/2 A D^-1/2, which has
+    the spectrum of D^-1 A, from the start vector v0:
+        v_1 = v0/||v0||;  w = S v_j - beta_{j-1} v_{j-1};  alpha_j = w.v_j;
+        w -= alpha_j v_j;  beta_j = ||w||;  v_{j+1} = w / beta_j.
+    (theta, s) = eigenpairs of tridiag(alpha, beta).  Every Ritz value lies inside the
+    spectrum and the residual norm of the Ritz pair (theta_max, V s) is beta_k |s_k| (s_k =
+    last component of s): an eigenvalue lies within that distance of theta_max, and
+    `upper` = theta_max + beta_k |s_k| is the usual safeguarded ESTIMATE of lam_max (not a
+    theorem: callers add a margin, the CUDA library 1 %); `upper_loose` = theta_max + beta_k.
+    Returns dict(theta_min, theta_max, beta_k, s_k, upper, upper_loose, steps)."""
+    from scipy.linalg import eigh_tridiagonal
+    ds = np.sqrt(np.asarray(dinv, dtype=np.float64)) if dinv is not None else None
+
+    def S(v):
+        t = v if ds is None else ds * v
+        t = apply_A(t[:, None])[:, 0]
+        return t if ds is None else ds * t
+
+    v = np.asarray(v0, dtype=np.float64).copy()
+    v /= np.linalg.norm(v)
+    v_prev = np.zeros_like(v)
+    alpha, beta = [], []
+    b = 0.0
+    for _j in range(k):
+        w = S(v) - b * v_prev
+        a = float(w @ v)
+        w = w - a * v
+        b = float(np.linalg.norm(w))
+        alpha.append(a)
+        beta.append(b)
+        if b <= 1e-300:
+            break
+        v_prev, v = v, w / b
+    if len(alpha) > 1:
+        theta, Sv = eigh_tridiagonal(np.array(alpha), np.array(beta[:-1]))
+    else:
+        theta, Sv = np.array(alpha), np.ones((1, 1))
+    s_k = float(abs(Sv[-1, -1]))
+    return dict(theta_min=float(theta[0]), theta_max=float(theta[-1]), beta_k=beta[-1], s_k=s_k,
+                upper=float(theta[-1]) + beta[-1] * s_k, upper_loose=float(theta[-1]) + beta[-1],
+                steps=len(alpha))
+
+
+def gershgorin_upper(A_dense, dinv=None):
+    """max_i d_i sum_j |a_ij| = ||D^-1 A||_inf >= every |eigenvalue| of D^-1 A."""
+    r = np.sum(np.abs(np.asarray(A_dense, dtype=np.float64)), axis=1)
+    return float(np.max(r if dinv is None else np.asarray(dinv) * r))
+
+
+def fe_cellwise_upper(A_cells, B_cell, cells=None):
+    """max over cells of lam_max(A_c, B_c) >= lam_max(A, B): x^T A x = sum_c x_c^T A_c x_c
+    <= max_c lam_max(A_c, B_c) sum_c x_c^T B_c x_c (mediant inequality; SURVEY reading S7).
+    `cells` = iterable of cell indices (all cells: rigorous; a sample: an estimate)."""
+    cells = range(A_cells.shape[0]) if cells is None else cells
+    n = B_cell.shape[0]
+    return max(float(sla.eigh(np.asarray(A_cells[c], dtype=np.float64), B_cell, eigvals_only=True,
+                              subset_by_index=[n - 1, n - 1])[0]) for c in cells)
 
 
 # --------------------------------------------------------------------------- diagnostics

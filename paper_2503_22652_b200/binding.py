@@ -14,6 +14,7 @@ OK, EINVAL, ENOMEM, ECUDA, ENOTCONVERGED, EBREAKDOWN = range(6)
 OP_DENSE, OP_CSR, OP_FE = 0, 1, 2
 FP64, FP32, TF32, BF16 = 0, 1, 2, 3
 METHOD_CHFSI, METHOD_RCHFSI = 0, 1
+USE_FILTER, USE_RAYLEIGH_RITZ, USE_SOLVE, USE_FILTER_HOST, USE_BOUNDS, USE_FILTER_NULL_G = 1, 2, 4, 8, 16, 32
 PREC = {"fp64": FP64, "fp32": FP32, "tf32": TF32, "bf16": BF16}
 STATUS_NAME = {0: "OK", 1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "ENOTCONVERGED", 5: "EBREAKDOWN"}
 
@@ -29,7 +30,13 @@ class RchfsiOptions(C.Structure):
     _fields_ = [("apply_prec", C.c_int32), ("store_prec", C.c_int32),
                 ("normalize_columns_before_rr", C.c_int32), ("adaptive_bounds", C.c_int32),
                 ("noise_eps", C.c_double), ("noise_seed", C.c_uint64),
-                ("g_input_f32", C.c_int32)]
+                ("allow_high_degree", C.c_int32), ("g_input_f32", C.c_int32)]
+
+
+class RchfsiBounds(C.Structure):
+    _fields_ = [("lam_max", C.c_double), ("lanczos_max", C.c_double), ("lanczos_theta_max", C.c_double),
+                ("lanczos_theta_min", C.c_double), ("gershgorin_max", C.c_double), ("fe_cellwise_max", C.c_double),
+                ("lanczos_steps", C.c_int32)]
 
 
 # every symbol include/rchfsi.h declares: name -> (restype, argtypes)
@@ -42,7 +49,10 @@ SYMBOLS = {
     "rchfsi_operator_changed": (C.c_int, [C.c_void_p]),
     "rchfsi_last_error": (C.c_char_p, [C.c_void_p]),
     "rchfsi_workspace_bytes": (C.c_size_t, [C.POINTER(RchfsiOperator), C.POINTER(RchfsiOperator), C.c_int32,
-                                            C.POINTER(RchfsiOptions)]),
+                                            C.POINTER(RchfsiOptions), C.c_int32, C.c_int32]),
+    "rchfsi_add_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
+    "rchfsi_workspace_shortfall": (C.c_size_t, [C.c_void_p]),
+    "rchfsi_workspace_used": (C.c_size_t, [C.c_void_p]),
     "rchfsi_filter": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                 C.c_double, C.c_double, C.c_double]),
     "rchfsi_filter_host": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
@@ -51,6 +61,7 @@ SYMBOLS = {
     "rchfsi_solve": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p,
                                C.POINTER(C.c_int32), C.c_void_p]),
+    "rchfsi_estimate_bounds": (C.c_int, [C.c_void_p, C.c_int32, C.c_int32, C.c_uint64, C.POINTER(RchfsiBounds)]),
     "rchfsi_apply": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
     "rchfsi_launch_count": (C.c_int64, [C.c_void_p]),
     "rchfsi_last_filter_step_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]),
@@ -133,11 +144,16 @@ def make_operator(spec, keep):
 
 
 class Rchfsi:
-    """Handle wrapper.  Method names mirror the C entry points (rchfsi_filter -> .filter, ...)."""
+    """Handle wrapper.  Method names mirror the C entry points (rchfsi_filter -> .filter, ...).
+
+    Device memory: the library allocates none.  `workspace=None` (default): torch tensors are handed to the handle
+    on demand -- a call that returns ENOMEM has not changed any caller block, so the binding adds a segment of
+    rchfsi_workspace_shortfall() bytes (torch.empty) and repeats the call.  `workspace=<uint8 CUDA tensor>`: that
+    single buffer only (size it with Rchfsi.workspace_bytes); running out raises."""
 
     def __init__(self, A, B=None, dinv=None, block_N=1, apply_prec="fp64", store_prec="fp64",
                  normalize_columns_before_rr=True, adaptive_bounds=False, noise_eps=0.0, noise_seed=0,
-                 g_input_f32=False, stream=None):
+                 allow_high_degree=False, g_input_f32=False, stream=None, workspace=None):
         import torch
         self.lib = load_library()
         self._keep = []
@@ -153,6 +169,7 @@ class Rchfsi:
         opt.adaptive_bounds = int(adaptive_bounds)
         opt.noise_eps = float(noise_eps)
         opt.noise_seed = int(noise_seed)
+        opt.allow_high_degree = int(allow_high_degree)
         opt.g_input_f32 = int(g_input_f32)
         self.opt = opt
         self.m, self.N = int(self.opA.m), int(block_N)
@@ -161,17 +178,63 @@ class Rchfsi:
         st = self.lib.rchfsi_create(C.byref(h), C.byref(self.opA),
                                     C.byref(self.opB) if self.opB is not None else None,
                                     _ptr(dinv), self.N, C.byref(opt), C.c_void_p(self.stream.cuda_stream))
-        if st != OK:
+        if st == ENOMEM or st == OK:
+            self.h = h
+        if st != OK and st != ENOMEM:
             raise RchfsiError(st, (self.lib.rchfsi_last_error(None) or b"").decode())
-        self.h = h
+        self._ws = []
+        self._grow = workspace is None
+        if workspace is not None:
+            _check_dev(workspace, torch.uint8, "workspace")
+            self.add_workspace(workspace)
+
+    @staticmethod
+    def workspace_bytes(A, B=None, block_N=1, uses=USE_FILTER, max_degree=64, **opts):
+        """rchfsi_workspace_bytes for operator specs as the constructor takes them."""
+        lib = load_library()
+        keep = []
+        opA = make_operator(A, keep)
+        opB = make_operator(B, keep) if B is not None else None
+        opt = RchfsiOptions()
+        lib.rchfsi_default_options(C.byref(opt))
+        for k, v in opts.items():
+            setattr(opt, k, PREC[v] if isinstance(v, str) else int(v))
+        return int(lib.rchfsi_workspace_bytes(C.byref(opA), C.byref(opB) if opB is not None else None, block_N,
+                                              C.byref(opt), uses, max_degree))
+
+    def add_workspace(self, t):
+        """rchfsi_add_workspace: hand a uint8 CUDA tensor to the handle (kept alive here)."""
+        st = self.lib.rchfsi_add_workspace(self.h, C.c_void_p(t.data_ptr()), t.numel())
+        if st != OK:
+            self._raise(st)
+        self._ws.append(t)
+
+    def workspace_used(self):
+        return int(self.lib.rchfsi_workspace_used(self.h))
+
+    def _call(self, fn, *args):
+        """Call an entry point; on ENOMEM (workspace exhausted, nothing of the caller's changed) add a torch-owned
+        segment of the missing size and repeat."""
+        import torch
+        while True:
+            st = fn(self.h, *args)
+            if st != ENOMEM or not self._grow:
+                return st
+            need = int(self.lib.rchfsi_workspace_shortfall(self.h))
+            if need <= 0:
+                return st
+            # small requests share a 1 MiB segment: fewer, larger torch tensors
+            self.add_workspace(torch.empty(max(need, 1 << 20), dtype=torch.uint8,
+                                           device=torch.device("cuda", torch.cuda.current_device())))
 
     def _raise(self, st):
         raise RchfsiError(st, (self.lib.rchfsi_last_error(self.h) or b"").decode())
 
     def close(self):
         if getattr(self, "h", None):
-            self.lib.rchfsi_destroy(self.h)
+            self.lib.rchfsi_destroy(self.h)     # synchronises the stream: the segments may go after it
             self.h = None
+            self._ws = []
 
     def __del__(self):
         try:
@@ -205,7 +268,7 @@ class Rchfsi:
                 self._block(G, "G")
         if ritz is not None:
             _check_dev(ritz, torch.float64, "ritz")
-        st = self.lib.rchfsi_filter(self.h, method, _ptr(X), _ptr(ritz), _ptr(G), degree, lam_min, lam_T, lam_max)
+        st = self._call(self.lib.rchfsi_filter, method, _ptr(X), _ptr(ritz), _ptr(G), degree, lam_min, lam_T, lam_max)
         if st != OK:
             self._raise(st)
         return X
@@ -232,9 +295,8 @@ class Rchfsi:
                                 (name, shape, "float32" if f32 else "float64"))
             return C.c_void_p(ptr)
         blk = (self.m, self.N)
-        st = self.lib.rchfsi_filter_host(self.h, method, hp(X_host, "X_host", blk), hp(ritz_host, "ritz_host", (self.N,)),
-                                         hp(G_host, "G_host", blk, f32=bool(self.opt.g_input_f32)), degree,
-                                         lam_min, lam_T, lam_max)
+        st = self._call(self.lib.rchfsi_filter_host, method, hp(X_host, "X_host", blk), hp(ritz_host, "ritz_host", (self.N,)),
+                        hp(G_host, "G_host", blk, f32=bool(self.opt.g_input_f32)), degree, lam_min, lam_T, lam_max)
         if st != OK:
             self._raise(st)
         return X_host
@@ -246,7 +308,7 @@ class Rchfsi:
         ritz = torch.empty(self.N, dtype=torch.float64, device=Y.device)
         res = torch.empty(self.N, dtype=torch.float64, device=Y.device)
         G = torch.empty_like(Y) if want_G else None
-        st = self.lib.rchfsi_rayleigh_ritz(self.h, _ptr(Y), _ptr(ritz), _ptr(G), _ptr(res))
+        st = self._call(self.lib.rchfsi_rayleigh_ritz, _ptr(Y), _ptr(ritz), _ptr(G), _ptr(res))
         if st != OK:
             self._raise(st)
         return ritz, Y, G, res
@@ -260,20 +322,28 @@ class Rchfsi:
         res = np.empty(self.N)
         hist = np.full(max_iter, np.nan)
         iters = C.c_int32(0)
-        st = self.lib.rchfsi_solve(self.h, method, _ptr(X), n_wanted, degree, lam_min, lam_T, lam_max, tol,
-                                   max_iter, C.c_void_p(evals.ctypes.data), C.c_void_p(res.ctypes.data),
-                                   C.byref(iters), C.c_void_p(hist.ctypes.data))
+        st = self._call(self.lib.rchfsi_solve, method, _ptr(X), n_wanted, degree, lam_min, lam_T, lam_max, tol,
+                        max_iter, C.c_void_p(evals.ctypes.data), C.c_void_p(res.ctypes.data),
+                        C.byref(iters), C.c_void_p(hist.ctypes.data))
         if st not in (OK, ENOTCONVERGED) or (st == ENOTCONVERGED and raise_on_not_converged):
             self._raise(st)
         return dict(evals=evals, resnorm=res, iters=iters.value, history=hist[:iters.value],
                     converged=(st == OK))
+
+    def estimate_bounds(self, lanczos_steps=20, fe_cell_stride=0, seed=0):
+        """rchfsi_estimate_bounds: dict of the estimates (lam_max = the recommended upper bound)."""
+        b = RchfsiBounds()
+        st = self._call(self.lib.rchfsi_estimate_bounds, lanczos_steps, fe_cell_stride, seed, C.byref(b))
+        if st != OK:
+            self._raise(st)
+        return {name: getattr(b, name) for name, _ in RchfsiBounds._fields_}
 
     def apply(self, which, V):
         """rchfsi_apply: exact FP64 A V (which=0) or B V (which=1)."""
         import torch
         self._block(V, "V")
         out = torch.empty_like(V)
-        st = self.lib.rchfsi_apply(self.h, which, _ptr(V), _ptr(out))
+        st = self._call(self.lib.rchfsi_apply, which, _ptr(V), _ptr(out))
         if st != OK:
             self._raise(st)
         return out

@@ -11,10 +11,12 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librchfsi.so")
 SOURCES = ["api.cu", "filter.cu", "kernels_simt.cu", "elementwise.cu", "rr.cu", "csr_fused.cu",
-           "dense_tc.cu", "fe_tc.cu", "fe_rr.cu"]
+           "dense_tc.cu", "fe_tc.cu", "fe_rr.cu", "bounds.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+if os.environ.get("RCHFSI_PROBES"):      # development build: timing probes (RCHFSI_TC_DEBUG) compiled in
+    FLAGS.append("-DRCHFSI_PROBES")
 
 
 def _stale():

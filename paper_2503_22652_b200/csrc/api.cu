@@ -1,6 +1,7 @@
 // C ABI of librchfsi.so (include/rchfsi.h): argument validation, workspace management and the
 // host-side control flow of Algorithms 1-3.  All arithmetic on blocks
 // runs in the CUDA kernels of this library; the host only computes the Chebyshev scalars.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -11,17 +12,25 @@ using namespace rchfsi;
 static thread_local std::string g_create_error;
 
 namespace rchfsi {
+// Every device buffer of a handle is carved from the caller's workspace segments (rchfsi_add_workspace): first fit,
+// 256-byte aligned, never returned (buffers live as long as the handle).  The library itself never calls cudaMalloc.
+constexpr size_t WS_ALIGN = 256;
 rchfsi_status dev_alloc(rchfsi_ctx *h, void **p, size_t bytes) {
-  void *q = nullptr;
-  cudaError_t e = cudaMalloc(&q, bytes ? bytes : 16);
-  if (e != cudaSuccess) {
-    cudaGetLastError();
-    h->err = "cudaMalloc(" + std::to_string(bytes) + " bytes): " + cudaGetErrorString(e);
-    return e == cudaErrorMemoryAllocation ? RCHFSI_ENOMEM : RCHFSI_ECUDA;
+  const size_t need = (std::max<size_t>(bytes, 16) + WS_ALIGN - 1) / WS_ALIGN * WS_ALIGN;
+  for (WorkspaceSegment &sg : h->segments) {
+    const size_t pad = (WS_ALIGN - (reinterpret_cast<uintptr_t>(sg.base) + sg.used) % WS_ALIGN) % WS_ALIGN;
+    if (sg.used + pad + need <= sg.size) {
+      *p = sg.base + sg.used + pad;
+      sg.used += pad + need;
+      h->ws_used += need;
+      h->shortfall = 0;
+      return RCHFSI_OK;
+    }
   }
-  h->owned.push_back(q);
-  *p = q;
-  return RCHFSI_OK;
+  h->shortfall = need + WS_ALIGN;
+  h->err = "workspace exhausted: a buffer of " + std::to_string(need) + " bytes does not fit (" + std::to_string(h->ws_used) +
+           " bytes in use); add a segment of rchfsi_workspace_shortfall() bytes with rchfsi_add_workspace and call again";
+  return RCHFSI_ENOMEM;
 }
 }  // namespace rchfsi
 
@@ -76,7 +85,6 @@ static Knobs read_knobs() {
   k.rr_timing = getenv("RCHFSI_RR_TIMING") != nullptr;
   k.rr_split = geti("RCHFSI_RR_SPLIT", -1);
   k.host_chunk = geti("RCHFSI_HOST_CHUNK", 0);
-  k.csr_variant = geti("RCHFSI_CSR_VARIANT", 0);
 #ifdef RCHFSI_PROBES
   k.tc_debug = geti("RCHFSI_TC_DEBUG", 0);
 #endif
@@ -138,7 +146,7 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const 
   }
   if (A->kind == RCHFSI_OP_FE) {
     // colouring of the cell conflict graph; also validates conn (range, every row covered by a cell)
-    rchfsi_status s = fe_ensure_coloring(h);
+    rchfsi_status s = fe_build_coloring(h);
     if (s != RCHFSI_OK) { g_create_error = h->err; rchfsi_destroy(h); return s; }
   }
   if (cudaEventCreate(&h->ev_step0) != cudaSuccess || cudaEventCreate(&h->ev_step1) != cudaSuccess) {
@@ -153,7 +161,6 @@ rchfsi_status rchfsi_create(rchfsi_handle *out, const rchfsi_operator *A, const 
 rchfsi_status rchfsi_destroy(rchfsi_handle h) {
   if (!h) return RCHFSI_EINVAL;
   cudaStreamSynchronize(h->stream);
-  for (void *p : h->owned) cudaFree(p);
   if (h->cublas) cublasDestroy(h->cublas);
   if (h->cusolver) cusolverDnDestroy(h->cusolver);
   for (int i = 0; i < rchfsi_ctx::HOST_SETS; ++i)
@@ -170,13 +177,8 @@ rchfsi_status rchfsi_destroy(rchfsi_handle h) {
 rchfsi_status rchfsi_operator_changed(rchfsi_handle h) {
   if (!h) return RCHFSI_EINVAL;
   RCHFSI_CUDA_CHECK(h, cudaStreamSynchronize(h->stream));
-  // the reduced-precision copies (with D^-1 folded in) and the TMA descriptors onto them are rebuilt on the next step
-  for (rchfsi::LowpCopy &c : h->lowp) {
-    for (size_t i = 0; i < h->owned.size(); ++i)
-      if (h->owned[i] == c.data) { h->owned.erase(h->owned.begin() + i); break; }
-    cudaFree(c.data);
-  }
-  h->lowp.clear();
+  // the reduced-precision copies (with D^-1 folded in) keep their buffers; their contents are rebuilt on the next step
+  for (rchfsi::LowpCopy &c : h->lowp) c.stale = true;
   h->tmaps.clear();
   return RCHFSI_OK;
 }
@@ -195,24 +197,64 @@ rchfsi_status rchfsi_last_filter_step_ms(rchfsi_handle h, float *ms_total_out, i
   return RCHFSI_OK;
 }
 
+rchfsi_status rchfsi_add_workspace(rchfsi_handle h, void *device_buffer, size_t bytes) {
+  if (!h) return RCHFSI_EINVAL;
+  if (!device_buffer || bytes < 2 * WS_ALIGN) { h->err = "rchfsi_add_workspace: null buffer or fewer than 512 bytes"; return RCHFSI_EINVAL; }
+  h->segments.push_back(rchfsi::WorkspaceSegment{static_cast<char *>(device_buffer), bytes, 0});
+  h->shortfall = 0;
+  return RCHFSI_OK;
+}
+
+size_t rchfsi_workspace_shortfall(rchfsi_handle h) { return h ? h->shortfall : 0; }
+size_t rchfsi_workspace_used(rchfsi_handle h) { return h ? h->ws_used : 0; }
+
+// Planner: the same buffers, by the same rules, as the allocation sites (ensure_filter_workspace, ensure_rr_workspace,
+// rchfsi_solve, rchfsi_filter_host, rchfsi_estimate_bounds, the reduced-precision operator copies), each rounded up
+// to the allocator's granule.  An upper bound that a single segment of this size satisfies; tests check both.
 size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B, int32_t block_N,
-                              const rchfsi_options *opt) {
+                              const rchfsi_options *opt, int32_t uses, int32_t max_degree) {
   if (!A || block_N < 1) return 0;
   rchfsi_options o;
   rchfsi_default_options(&o);
   if (opt) o = *opt;
-  const size_t el = (size_t)A->m * block_N;
-  const size_t s = prec_bytes(o.store_prec);
-  size_t total = 2 * el * s;                              // R_X, R_Y
-  if (o.store_prec != RCHFSI_FP64) total += el * s;       // storage-precision copy of G
-  total += 2 * el * 4;                                    // operand shadows (worst case FP32)
-  total += el * 8;                                        // unfused operator output / G scratch
-  total += (B ? 3 : 2) * el * 8 + el * 8;                 // Rayleigh-Ritz temporaries + solve's G
-  total += 2 * (size_t)block_N * block_N * 8 * 2;         // Gram matrices + dsygvd workspace (approx.)
-  if (A->kind == RCHFSI_OP_DENSE && o.apply_prec != RCHFSI_FP64) total += (size_t)A->m * A->m * 4;
-  if (A->kind == RCHFSI_OP_FE && o.apply_prec != RCHFSI_FP64)
-    total += (size_t)A->n_cells * 352 * 352 * (o.apply_prec == RCHFSI_BF16 ? 2 : 4);
-  if (A->kind == RCHFSI_OP_FE) total += (size_t)1600 << 20;   // gather / product / FP64 cell-batch scratch of the Rayleigh-Ritz applies
+  const Knobs kn = read_knobs();
+  const Plan pl = make_plan(*A, block_N, o, kn);
+  const size_t m = (size_t)A->m, N = (size_t)block_N;
+  auto al = [](size_t b) { return (std::max<size_t>(b, 16) + WS_ALIGN - 1) / WS_ALIGN * WS_ALIGN + WS_ALIGN; };
+  size_t total = 0;
+  const size_t el = m * N, el_lib = m * (pl.panel ? (size_t)cdiv(block_N, 128) * 128 : N);
+  const bool fe = A->kind == RCHFSI_OP_FE;
+  if (fe) total += al(4 * (size_t)A->n_cells) + al((size_t)A->n_cells * A->n_loc);            // colouring: cell order + flags
+  const bool want_filter = uses & (RCHFSI_USE_FILTER | RCHFSI_USE_SOLVE | RCHFSI_USE_FILTER_HOST);
+  if (want_filter) {
+    total += 2 * al(el_lib * prec_bytes(pl.store));                                           // R_X, R_Y
+    if (pl.shadow) total += (pl.shadow_inplace ? 1 : 2) * al(el_lib * (pl.operand == RCHFSI_BF16 ? 2 : 4));
+    if (pl.fused == 0) total += al(el_lib * prec_bytes(pl.tprec));                            // unfused operator output
+    if (!o.g_input_f32 && (pl.store != RCHFSI_FP64 || pl.panel)) total += al(el_lib * prec_bytes(pl.store));   // G in storage layout
+    total += al(8 * (size_t)(std::max(max_degree, 1) + 1) * N) + al(16 * N);                  // Lambda_k table, column norms
+    if (uses & RCHFSI_USE_FILTER_NULL_G) total += 2 * al(el * 8);                             // G = NULL: A X and G in FP64
+    // reduced-precision operator copies: with and without D^-1 folded in (R-ChFSI / ChFSI)
+    size_t lp = 0;
+    if (pl.fused == 1) lp = al(csr_lowp_bytes(*A));
+    if (pl.fused == 2) lp = al(dense_lowp_bytes(*A, o.apply_prec));
+    if (pl.fused == 3) lp = al(fe_lowp_bytes(*A, o.apply_prec));
+    total += 2 * lp;
+  }
+  if (uses & (RCHFSI_USE_RAYLEIGH_RITZ | RCHFSI_USE_SOLVE)) {
+    total += (B ? 3 : 2) * al(el * 8);                                                        // A Y, (B Y), rotation target
+    total += 2 * al(8 * N * N) + 2 * al(8 * N) + al(16 * N) + al(4);                          // Gram matrices, Ritz values, residuals
+    total += al(8 * (2 * N * N + 8 * N + 64) + (size_t)1 << 20);                              // dsygvd workspace (cuSOLVER query at run time)
+    if (fe) total += fe_rr_scratch_bytes(*A, block_N, A->n_cells);
+  }
+  if (uses & RCHFSI_USE_SOLVE) total += al(el * 8);                                           // residual block of the solve
+  if (uses & RCHFSI_USE_FILTER_HOST) {
+    const size_t gb = o.g_input_f32 ? 4 : 8;
+    total += 3 * (al(el * 8) + al(el * gb)) + al(8 * N);                                      // at most the whole block per staging set
+  }
+  if (uses & RCHFSI_USE_BOUNDS) {
+    total += al(8 * (5 * m + 4));
+    if (fe) total += al(8 * (2 * (size_t)A->n_loc * A->n_loc + A->n_loc + 2)) + al(8 * (3 * (size_t)A->n_loc * A->n_loc + 64 * (size_t)A->n_loc) + ((size_t)1 << 20));
+  }
   return total;
 }
 

@@ -32,6 +32,7 @@ struct StepCoef {
 struct LowpCopy {
   int prec = -1;          // RCHFSI_TF32 / RCHFSI_BF16 / RCHFSI_FP32
   bool folded = false;    // columns pre-scaled by dinv (A * diag(dinv))
+  bool stale = false;     // rchfsi_operator_changed: the buffer stays, its contents are rebuilt on the next use
   void *data = nullptr;   // dense: [m_pad][k_pad]; FE: [n_cells][a_pad][k_pad]
   int64_t ld = 0;         // padded K extent (elements)
   int64_t rows_pad = 0;   // padded row extent per matrix
@@ -58,9 +59,29 @@ struct Knobs {
   bool rr_fe_simt = false;       // RCHFSI_RR_FE_SIMT: FE applies of the Rayleigh-Ritz through the hand-written FP64 kernel
   bool rr_timing = false;        // RCHFSI_RR_TIMING: print phase times of the Rayleigh-Ritz to stderr
   int rr_split = -1;             // RCHFSI_RR_SPLIT: Gram / rotation products on the tensor pipe (split operands), -1 = automatic
-  int csr_variant = 0;           // RCHFSI_CSR_VARIANT: tuning sweep of the fused CSR step (0 = round-1 kernel)
   int host_chunk = 0;            // RCHFSI_HOST_CHUNK: column-chunk width of rchfsi_filter_host (multiple of 128), 0 = automatic
   int tc_debug = 0;              // RCHFSI_TC_DEBUG (only in -DRCHFSI_PROBES builds)
+};
+
+// How rchfsi_filter lays out its blocks for (operator, block width, options): which fused kernel runs, which
+// precision the operand block has, whether an operand shadow exists.  Decided from the descriptor alone so that
+// rchfsi_workspace_bytes can plan without a handle.
+struct Plan {
+  int store;     // storage precision of R_X, R_Y, G
+  int operand;   // precision of the block the operator kernel reads
+  int tprec;     // precision of the unfused operator output T
+  bool shadow;   // operand block is a separate buffer
+  int fused;     // 0 unfused SIMT, 1 CSR fused, 2 dense tensor-core, 3 FE tensor-core
+  bool panel;    // library-owned blocks in panel layout [ceil(N/128)][m][128] (FE tensor-core path)
+  bool shadow_inplace;   // one shadow buffer, overwritten in place by the fused FE step
+};
+struct Knobs;
+Plan make_plan(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt, const Knobs &kn);
+
+// A piece of caller-provided device memory the handle carves its buffers from (rchfsi_add_workspace)
+struct WorkspaceSegment {
+  char *base;
+  size_t size, used;
 };
 
 struct DeviceOperator {
@@ -74,6 +95,8 @@ struct FeColoring {
   std::vector<int64_t> color_begin;   // [n_colors + 1] into cell_order
   int32_t *cell_order = nullptr;      // device [n_cells], cells grouped by colour
   uint8_t *flags = nullptr;           // device [n_cells][n_loc]: bit0 first toucher, bit1 last toucher
+  std::vector<int32_t> h_order;       // host copies, built (and the mesh validated) in rchfsi_create; uploaded into the
+  std::vector<uint8_t> h_flags;       // workspace on first use
 };
 
 }  // namespace rchfsi
@@ -114,7 +137,7 @@ struct rchfsi_ctx {
   float *Gsolve32 = nullptr;                               // [m][N] FP32 residual block of rchfsi_solve (chunked mode)
   double *feg_W = nullptr, *feg_T = nullptr, *feg_A = nullptr;  // fe_rr.cu scratch: gathered operand, product, FP64 cell batch
   const double **feg_ptrs = nullptr;                        // [3][feg_ptr_cap] pointer arrays of the batched GEMM
-  size_t feg_w_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0;
+  size_t feg_w_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0; int32_t feg_N = 0;
   double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
@@ -133,11 +156,18 @@ struct rchfsi_ctx {
   cudaEvent_t ev_x = nullptr;              // the X event the running filter has to wait for (one of ev_xin)
   bool x_pending = false;
 
+  // rchfsi_estimate_bounds scratch (bounds.cu)
+  double *bnd_buf = nullptr, *bnd_cell = nullptr, *bnd_work = nullptr;
+
   // instrumentation
   cudaEvent_t ev_step0 = nullptr, ev_step1 = nullptr;
   int32_t last_steps = 0;
 
-  std::vector<void *> owned;   // everything cudaMalloc'ed by this handle
+  // caller-provided workspace (rchfsi_add_workspace): every device buffer of the handle is carved from these
+  // segments; the library itself never calls cudaMalloc
+  std::vector<rchfsi::WorkspaceSegment> segments;
+  size_t shortfall = 0;        // bytes of the allocation that did not fit (rchfsi_workspace_shortfall)
+  size_t ws_used = 0;          // bytes handed out so far
 };
 
 namespace rchfsi {
@@ -245,15 +275,22 @@ struct FusedStep {
   bool chfsi;           // dinv applied to the output rows instead of the input
   bool g_rowmajor;      // G is the caller's row-major [m][N] block even though R_X / R_Y use the panel layout
 };
-bool csr_fused_supported(const rchfsi_ctx *h);
+bool csr_fused_supported(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt);
 rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s);
-bool dense_tc_supported(const rchfsi_ctx *h);
+bool dense_tc_supported(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt);
 rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s);
-bool fe_tc_supported(const rchfsi_ctx *h);
+bool fe_tc_supported(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt);
+// bytes of the reduced-precision operator copy each fused path keeps (0 when the path does not apply)
+size_t csr_lowp_bytes(const rchfsi_operator &A);
+size_t dense_lowp_bytes(const rchfsi_operator &A, int prec);
+size_t fe_lowp_bytes(const rchfsi_operator &A, int prec);
+// scratch of the batched-GEMM FE applies of the Rayleigh-Ritz for an N-column block
+size_t fe_rr_scratch_bytes(const rchfsi_operator &op, int32_t N, int64_t max_cells_per_colour);
 rchfsi_status fe_tc_step(rchfsi_ctx *h, const FusedStep &s);
 
 // ---- fe_rr.cu / fe_tc.cu ---------------------------------------------------------------
-rchfsi_status fe_ensure_coloring(rchfsi_ctx *h);
+rchfsi_status fe_build_coloring(rchfsi_ctx *h);    // host side: colours, order, flags; validates conn (create time)
+rchfsi_status fe_ensure_coloring(rchfsi_ctx *h);   // device side: uploads order and flags into the workspace (first use)
 bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op);
 // T = Op W in FP64 through gather -> batched DGEMM -> coloured scatter (Rayleigh-Ritz only)
 rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,

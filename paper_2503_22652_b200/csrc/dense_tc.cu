@@ -395,24 +395,32 @@ __global__ void dense_lowp_kernel(const double *__restrict__ A, int64_t lda, con
 
 const LowpCopy *get_dense_copy(rchfsi_ctx *h, int prec, bool folded, rchfsi_status *st) {
   *st = RCHFSI_OK;
-  for (const LowpCopy &c : h->lowp)
-    if (c.prec == prec && c.folded == folded) return &c;
-  LowpCopy c;
-  c.prec = prec;
-  c.folded = folded;
-  c.ld = cdiv(h->m, 64) * 64;
-  c.rows_pad = h->m;
-  c.bytes = (size_t)h->m * c.ld * (prec == RCHFSI_BF16 ? 2 : 4);
-  *st = dev_alloc(h, &c.data, c.bytes);
-  if (*st != RCHFSI_OK) return nullptr;
-  const unsigned grid = (unsigned)std::min<int64_t>(cdiv(h->m * c.ld, 256), 148 * 16);
-  if (prec == RCHFSI_BF16)
-    dense_lowp_kernel<1><<<grid, 256, 0, h->stream>>>(h->A.d.dense, h->A.d.lda, folded ? h->dinv : nullptr, c.data, h->m, c.ld);
-  else
-    dense_lowp_kernel<0><<<grid, 256, 0, h->stream>>>(h->A.d.dense, h->A.d.lda, folded ? h->dinv : nullptr, c.data, h->m, c.ld);
-  h->launches++;
-  h->lowp.push_back(c);
-  return &h->lowp.back();
+  LowpCopy *cp = nullptr;
+  for (LowpCopy &c : h->lowp)
+    if (c.prec == prec && c.folded == folded) cp = &c;
+  if (!cp) {
+    LowpCopy c;
+    c.prec = prec;
+    c.folded = folded;
+    c.stale = true;
+    c.ld = cdiv(h->m, 64) * 64;
+    c.rows_pad = h->m;
+    c.bytes = dense_lowp_bytes(h->A.d, prec);
+    *st = dev_alloc(h, &c.data, c.bytes);
+    if (*st != RCHFSI_OK) return nullptr;
+    h->lowp.push_back(c);
+    cp = &h->lowp.back();
+  }
+  if (cp->stale) {
+    const unsigned grid = (unsigned)std::min<int64_t>(cdiv(h->m * cp->ld, 256), 148 * 16);
+    if (prec == RCHFSI_BF16)
+      dense_lowp_kernel<1><<<grid, 256, 0, h->stream>>>(h->A.d.dense, h->A.d.lda, folded ? h->dinv : nullptr, cp->data, h->m, cp->ld);
+    else
+      dense_lowp_kernel<0><<<grid, 256, 0, h->stream>>>(h->A.d.dense, h->A.d.lda, folded ? h->dinv : nullptr, cp->data, h->m, cp->ld);
+    h->launches++;
+    cp->stale = false;
+  }
+  return cp;
 }
 
 template <int KIND, int BN, typename S>
@@ -448,11 +456,14 @@ rchfsi_status launch_dense_bn(rchfsi_ctx *h, int bn, const CUtensorMap &tmW, con
 
 }  // namespace
 
-bool dense_tc_supported(const rchfsi_ctx *h) {
-  if (h->A.d.kind != RCHFSI_OP_DENSE) return false;
-  if (h->opt.apply_prec == RCHFSI_TF32) return h->N % 4 == 0;
-  if (h->opt.apply_prec == RCHFSI_BF16) return h->N % 8 == 0;
+bool dense_tc_supported(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt) {
+  if (A.kind != RCHFSI_OP_DENSE) return false;
+  if (opt.apply_prec == RCHFSI_TF32) return N % 4 == 0;
+  if (opt.apply_prec == RCHFSI_BF16) return N % 8 == 0;
   return false;
+}
+size_t dense_lowp_bytes(const rchfsi_operator &A, int prec) {
+  return (size_t)A.m * (size_t)(cdiv(A.m, 64) * 64) * (prec == RCHFSI_BF16 ? 2 : 4);
 }
 
 // Tile height BN (operator rows per CTA) and K splits.  Large problems: the widest tile that still gives a full

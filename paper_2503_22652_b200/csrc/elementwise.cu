@@ -2,7 +2,9 @@
 // paths, plus the small reductions (column norms, residual norms) and the debug noise hook.
 // Blocks are [m][N] row-major; storage precision is a run-time code (RCHFSI_FP64 / FP32 /
 // BF16) handled by uniform branches: these kernels are HBM-bound.
+#include <mutex>
 #include "common.cuh"
+#include "rng.cuh"
 
 namespace rchfsi {
 
@@ -357,20 +359,6 @@ rchfsi_status symmetrize(rchfsi_ctx *h, double *H, int32_t N) {
 // Counter-based N(0,1): splitmix64 of (seed, apply index, i*N + j), Box-Muller.  The same map
 // is implemented by workloads/noise.py (the random numbers are an INPUT of the inexact
 // operator, reading S11).
-__device__ __forceinline__ uint64_t splitmix64(uint64_t x) {
-  x += 0x9E3779B97F4A7C15ull;
-  uint64_t z = x;
-  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-  return z ^ (z >> 31);
-}
-__device__ __forceinline__ double counter_gauss(uint64_t base, uint64_t idx) {
-  const uint64_t k1 = splitmix64(base + idx);
-  const uint64_t k2 = splitmix64(k1);
-  const double u1 = ((double)(k1 >> 11) + 0.5) * (1.0 / 9007199254740992.0);
-  const double u2 = ((double)(k2 >> 11) + 0.5) * (1.0 / 9007199254740992.0);
-  return sqrt(-2.0 * log(u1)) * cos(2.0 * 3.14159265358979323846 * u2);
-}
 __global__ void __launch_bounds__(256) noise_norm_kernel(const void *T, int prec, int64_t m, int32_t N,
                                                          int64_t rows_per_cta, uint64_t base, double *tn2,
                                                          double *gn2) {
@@ -400,17 +388,9 @@ __global__ void __launch_bounds__(256) noise_add_kernel(void *T, int prec, int64
   }
 }
 
-static uint64_t host_splitmix64(uint64_t x) {
-  x += 0x9E3779B97F4A7C15ull;
-  uint64_t z = x;
-  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-  return z ^ (z >> 31);
-}
-
 rchfsi_status add_column_noise(rchfsi_ctx *h, int t_prec, void *T, int64_t m, int32_t N, double eps,
                                uint64_t seed, uint64_t apply_index, double *scratch2N) {
-  const uint64_t base = host_splitmix64(seed ^ (apply_index * 0xD1B54A32D192ED03ull));
+  const uint64_t base = splitmix64(seed ^ (apply_index * 0xD1B54A32D192ED03ull));
   RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(scratch2N, 0, sizeof(double) * 2 * N, h->stream));
   int64_t ctas = std::min<int64_t>(m, 148 * 8);
   int64_t rows = cdiv(m, ctas);
@@ -442,9 +422,15 @@ __global__ void fe_asym_kernel(const TM *mats, int64_t n_mats, int32_t n_loc, do
   atomicMax(reinterpret_cast<unsigned long long *>(out), (unsigned long long)__double_as_longlong(worst));
 }
 
+// result cell of the symmetry check: module-scope device memory (rchfsi_create runs before any workspace exists and
+// the library never calls cudaMalloc); creates are serialised on it
+__device__ double g_asym_cell;
+static std::mutex g_asym_mutex;
+
 rchfsi_status fe_check_symmetric(rchfsi_ctx *h, const rchfsi_operator &op, double *max_asym_host) {
+  std::lock_guard<std::mutex> lock(g_asym_mutex);
   double *d = nullptr;
-  RCHFSI_CUDA_CHECK(h, cudaMalloc(&d, sizeof(double)));
+  RCHFSI_CUDA_CHECK(h, cudaGetSymbolAddress((void **)&d, g_asym_cell));
   cudaMemsetAsync(d, 0, sizeof(double), h->stream);
   const int64_t n_mats = op.cell_shared ? 1 : op.n_cells;
   if (op.cell_mats)
@@ -454,7 +440,6 @@ rchfsi_status fe_check_symmetric(rchfsi_ctx *h, const rchfsi_operator &op, doubl
   h->launches++;
   cudaError_t e = cudaMemcpyAsync(max_asym_host, d, sizeof(double), cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-  cudaFree(d);
   if (e != cudaSuccess) {
     h->err = std::string("fe_check_symmetric: ") + cudaGetErrorString(e);
     return RCHFSI_ECUDA;

@@ -87,6 +87,21 @@ __global__ void feg_pointers_kernel(const double **ptrs, int64_t batch, int64_t 
 
 }  // namespace
 
+// cells per batched-GEMM call: one colour at most, about 1.5 GB of scratch at most
+static int64_t fe_rr_cells_per_batch(const rchfsi_operator &op, int32_t N, int64_t max_color) {
+  const int32_t nl = op.n_loc;
+  const bool conv = (op.cell_mats == nullptr);
+  const size_t per_cell = 2 * sizeof(double) * (size_t)nl * N + (conv ? sizeof(double) * (size_t)nl * nl : 0);
+  return std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(max_color, (int64_t)(1.5e9 / (double)per_cell)), ((int64_t)1 << 30) / nl));
+}
+size_t fe_rr_scratch_bytes(const rchfsi_operator &op, int32_t N, int64_t max_color) {
+  if (op.kind != RCHFSI_OP_FE) return 0;
+  const int64_t cap = fe_rr_cells_per_batch(op, N, max_color);
+  const int32_t nl = op.n_loc;
+  return 2 * (sizeof(double) * (size_t)cap * nl * N + 256) + (op.cell_mats == nullptr ? sizeof(double) * (size_t)cap * nl * nl + 256 : 0) +
+         sizeof(double *) * 3 * (size_t)cap + 256;
+}
+
 bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op) {
   if (h->knobs.rr_fe_simt) return false;                               // A/B knob: keep the hand-written kernel
   const rchfsi_operator &A = h->A.d;
@@ -103,12 +118,14 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   const int32_t nl = op.n_loc;
   const bool conv = (op.cell_mats == nullptr);
   const int64_t mper = op.cell_shared ? 0 : (int64_t)nl * nl;
-  // scratch: gathered operand + product (+ FP64 copy of FP32 cell matrices), about 1.5 GB
-  const size_t per_cell = 2 * sizeof(double) * (size_t)nl * N + (conv ? sizeof(double) * (size_t)nl * nl : 0);
+  // scratch: gathered operand + product (+ FP64 copy of FP32 cell matrices), about 1.5 GB; sized once for the widest
+  // block the handle can see (N_cap or the chunk width of the memory-light Rayleigh-Ritz)
   int64_t max_color = 0;
   for (int k = 0; k < col.n_colors; ++k) max_color = std::max(max_color, col.color_begin[k + 1] - col.color_begin[k]);
-  const int64_t cap = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(max_color, (int64_t)(1.5e9 / (double)per_cell)), ((int64_t)1 << 30) / nl));
-  const size_t need_w = sizeof(double) * (size_t)cap * nl * N;
+  const int32_t Nw = std::max<int32_t>(N, h->feg_N);
+  const int64_t cap = fe_rr_cells_per_batch(op, Nw, max_color);
+  const size_t need_w = sizeof(double) * (size_t)cap * nl * Nw;
+  h->feg_N = Nw;
   if (h->feg_w_bytes < need_w) {
     RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_W, need_w));
     RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_T, need_w));

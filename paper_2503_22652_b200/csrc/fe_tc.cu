@@ -17,6 +17,7 @@
 // exact identity A D^-1 = sum_c P_c^T (A_c D_c^-1) P_c.
 #include <algorithm>
 #include <cstdlib>
+#include <type_traits>
 #include "common.cuh"
 #include "tc_common.cuh"
 

@@ -7,31 +7,21 @@
 
 using namespace rchfsi;
 
-namespace {
+namespace rchfsi {
 
-struct Plan {
-  int store;     // storage precision of R_X, R_Y, G
-  int operand;   // precision of the block the operator kernel reads
-  int tprec;     // precision of the unfused operator output T
-  bool shadow;   // operand block is a separate buffer
-  int fused;     // 0 unfused SIMT, 1 CSR fused, 2 dense tensor-core, 3 FE tensor-core
-  bool panel;    // library-owned blocks in panel layout [ceil(N/128)][m][128] (FE tensor-core path)
-  bool shadow_inplace;   // one shadow buffer, overwritten in place by the fused FE step (see make_plan)
-};
-
-Plan make_plan(const rchfsi_ctx *h) {
+Plan make_plan(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt, const Knobs &kn) {
   Plan p{};
-  p.store = h->opt.store_prec;
-  const int ap = h->opt.apply_prec;
+  p.store = opt.store_prec;
+  const int ap = opt.apply_prec;
   p.fused = 0;
   if (ap == RCHFSI_FP64) {
     p.operand = RCHFSI_FP64;
   } else {
     p.operand = RCHFSI_FP32;
-    if (h->opt.noise_eps <= 0) {
-      if (h->A.d.kind == RCHFSI_OP_CSR && csr_fused_supported(h)) p.fused = 1;
-      if (h->A.d.kind == RCHFSI_OP_DENSE && ap != RCHFSI_FP32 && dense_tc_supported(h)) p.fused = 2;
-      if (h->A.d.kind == RCHFSI_OP_FE && ap != RCHFSI_FP32 && fe_tc_supported(h)) p.fused = 3;
+    if (opt.noise_eps <= 0) {
+      if (A.kind == RCHFSI_OP_CSR && csr_fused_supported(A, N, opt)) p.fused = 1;
+      if (A.kind == RCHFSI_OP_DENSE && ap != RCHFSI_FP32 && dense_tc_supported(A, N, opt)) p.fused = 2;
+      if (A.kind == RCHFSI_OP_FE && ap != RCHFSI_FP32 && fe_tc_supported(A, N, opt)) p.fused = 3;
     }
     if (p.fused >= 2 && ap == RCHFSI_BF16) p.operand = RCHFSI_BF16;
     if (p.fused == 1) p.operand = p.store;   // the CSR kernel reads R_Y itself, converting on the fly
@@ -45,9 +35,15 @@ Plan make_plan(const rchfsi_ctx *h) {
   // before its epilogue starts: the new shadow may overwrite the old one, one buffer instead of two
   // (14.8 GB instead of 29.6 GB of BF16 shadows at config 5).  The dense step cannot: its row tiles read all rows.
   // RCHFSI_FE_SHADOW_PAIR=1 keeps the two-buffer scheme (the tests compare the two bit for bit).
-  p.shadow_inplace = p.shadow && p.fused == 3 && !h->knobs.fe_shadow_pair;
+  p.shadow_inplace = p.shadow && p.fused == 3 && !kn.fe_shadow_pair;
   return p;
 }
+
+}  // namespace rchfsi
+
+namespace {
+
+Plan make_plan(const rchfsi_ctx *h) { return rchfsi::make_plan(h->A.d, h->N, h->opt, h->knobs); }
 
 rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t degree, bool need_gs) {
   // sized for the block width of rchfsi_create (N_cap), whatever the active width of this call
@@ -105,6 +101,11 @@ static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, con
   if (method == RCHFSI_METHOD_RCHFSI && !ritz) { h->err = "rchfsi_filter: ritz is required for R-ChFSI"; return RCHFSI_EINVAL; }
   if (G && (reinterpret_cast<uintptr_t>(G) & 15u)) { h->err = "rchfsi_filter: G misaligned"; return RCHFSI_EINVAL; }
   if (degree < 1) { h->err = "rchfsi_filter: degree < 1"; return RCHFSI_EINVAL; }
+  if (degree >= 100 && h->opt.apply_prec != RCHFSI_FP64 && !h->opt.allow_high_degree) {
+    // PAPER.md:347-359 and footnote 5: FP32 / TF32 R-ChFSI matches FP64 for p <= 80, not for p = 100, 120
+    h->err = "rchfsi_filter: degree >= 100 with a reduced-precision apply is unstable (PAPER.md:347-359); set allow_high_degree to force it";
+    return RCHFSI_EINVAL;
+  }
   if (!(lam_min < lam_T) || !(lam_T < lam_max) || !std::isfinite(lam_min) || !std::isfinite(lam_max)) {
     h->err = "rchfsi_filter: need lam_min < lam_T < lam_max";
     return RCHFSI_EINVAL;

@@ -2,6 +2,7 @@
 // Off the hot path: the Gram and rotation products are plain library
 // GEMMs (cuBLAS dgemm) and the N x N generalized eigenproblem is cuSOLVER dsygvd; the operator
 // applies are this library's FP64 kernels.
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include "common.cuh"
@@ -150,6 +151,7 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
   }
   pt.lap("normalise columns");
   double *AY = h->rr1;
+  h->feg_N = std::max(h->feg_N, N);     // FE apply scratch sized once for the whole block
   RCHFSI_TRY(apply64(h, h->A.d, Y, AY, N));
   pt.lap("A Y");
   const double *BY = Y;
@@ -239,6 +241,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)rp * N));
   }
   const int32_t cw = h->rr_cw;
+  h->feg_N = std::max(h->feg_N, cw);    // FE apply scratch sized once for the chunk width
   const double one = 1.0, zero = 0.0;
   PhaseTimer pt(h);
   if (h->opt.normalize_columns_before_rr) {

@@ -114,6 +114,18 @@ __device__ __forceinline__ void st_global_u16(uint64_t addr, uint16_t v) { asm v
 __device__ __forceinline__ void cp_async16_sa(uint32_t smem_dst, uint64_t gsrc, uint32_t src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
 }
+// shared-memory loads addressed by a 32-bit shared-window address (LDS with an immediate offset, no generic math)
+template <typename S> __device__ __forceinline__ S lds_s(uint32_t saddr);
+template <> __device__ __forceinline__ float lds_s<float>(uint32_t saddr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(saddr));
+  return v;
+}
+template <> __device__ __forceinline__ double lds_s<double>(uint32_t saddr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(saddr));
+  return v;
+}
 // the mbarrier receives one arrival from this thread when all its earlier cp.async have landed
 // (.noinc: the arrival is part of the barrier's expected count)
 __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t *bar) {

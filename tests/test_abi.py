@@ -73,7 +73,11 @@ def test_null_handle_is_einval_everywhere():
     assert lib.rchfsi_apply(None, 0, None, None) == P.EINVAL
     assert lib.rchfsi_destroy(None) == P.EINVAL
     assert lib.rchfsi_launch_count(None) == -1
-    assert lib.rchfsi_workspace_bytes(None, None, 4, None) == 0
+    assert lib.rchfsi_workspace_bytes(None, None, 4, None, P.USE_FILTER, 10) == 0
+    assert lib.rchfsi_add_workspace(None, None, 0) == P.EINVAL
+    assert lib.rchfsi_workspace_shortfall(None) == 0 and lib.rchfsi_workspace_used(None) == 0
+    assert lib.rchfsi_operator_changed(None) == P.EINVAL
+    assert lib.rchfsi_estimate_bounds(None, 10, 0, 0, None) == P.EINVAL
 
 
 def test_no_cpu_fallback_without_a_device():
@@ -92,6 +96,18 @@ def test_workspace_bytes_scales_with_the_block():
     lib = P.load_library()
     op = P.RchfsiOperator()
     op.kind, op.m, op.dense, op.lda = P.OP_DENSE, 1000, 4096, 1000
-    a = lib.rchfsi_workspace_bytes(C.byref(op), None, 60, None)
-    b = lib.rchfsi_workspace_bytes(C.byref(op), None, 120, None)
-    assert 1000 * 60 * 8 * 4 < a < b
+    a = lib.rchfsi_workspace_bytes(C.byref(op), None, 60, None, P.USE_FILTER, 20)
+    b = lib.rchfsi_workspace_bytes(C.byref(op), None, 120, None, P.USE_FILTER, 20)
+    assert 1000 * 60 * 8 * 3 <= a < b       # R_X, R_Y and the unfused operator output
+    # more entry points need more; the plan needs no device
+    c = lib.rchfsi_workspace_bytes(C.byref(op), None, 60, None, P.USE_FILTER | P.USE_SOLVE, 20)
+    d = lib.rchfsi_workspace_bytes(C.byref(op), None, 60, None, P.USE_FILTER | P.USE_SOLVE | P.USE_FILTER_HOST | P.USE_BOUNDS, 20)
+    assert a < c < d
+    # configs[4] as BASELINE.json states it: the filter-only plan fits one B200 next to X (58.5 GB) and G (29.3 GB)
+    fe = P.RchfsiOperator()
+    fe.kind, fe.m, fe.n_cells, fe.n_loc, fe.conn, fe.cell_mats_f32 = P.OP_FE, 145 ** 3, 24 ** 3, 343, 4096, 4096
+    opt = P.RchfsiOptions()
+    lib.rchfsi_default_options(C.byref(opt))
+    opt.apply_prec, opt.store_prec, opt.g_input_f32 = P.BF16, P.FP32, 1
+    w5 = lib.rchfsi_workspace_bytes(C.byref(fe), None, 2400, C.byref(opt), P.USE_FILTER, 50)
+    assert 75e9 < w5 < (180e9 - 58.6e9 - 29.3e9)

@@ -465,3 +465,59 @@ def test_config1_noise_rchfsi_reaches_tol_chfsi_floors():
     assert rc["history"][-1] < 1e-8
     assert ch["history"][-1] > 1e-7
     np.testing.assert_allclose(rc["evals"][:20], cfg["lam"][:20], atol=1e-9)
+
+
+# ----------------------------------------------------------------------------- spectral-bound estimators (NEXT-4)
+def test_bounds_lanczos_is_the_krylov_projection_and_brackets_lam_max():
+    """lanczos_upper_bound against what the mathematics fixes: (i) the Ritz values equal the eigenvalues of the
+    projection Q^T S Q onto an orthonormal basis of the Krylov space span{v0, S v0, ..} built independently by QR
+    (textbook definition of the Lanczos Ritz values); (ii) with the exact spectrum from a dense eigensolver:
+    theta_max <= lam_max (Ritz values lie inside the spectrum), an eigenvalue lies within the residual norm
+    beta_k |s_k| of theta_max (residual theorem for symmetric matrices), and the safeguarded estimate with the
+    library's 1 % margin, 1.01 (theta_max + beta_k |s_k|), is above lam_max for several start vectors and k;
+    (iii) run to k = m on a tiny matrix it returns the exact extreme eigenvalues."""
+    prob = W.fe_problem(2, q=3, seed=9)
+    A, B, Dinv = O.operators_from_workload(prob)
+    m, d = prob["m"], prob["dinv"]
+    Ad = A.apply(np.eye(m))
+    s = np.sqrt(d)
+    S = s[:, None] * Ad * s[None, :]
+    lam = np.linalg.eigvalsh(S)
+    v0 = W.counter_gaussian(5, 0, m, 1)[:, 0]
+    k = 12
+    r = O.lanczos_upper_bound(A.apply, d, v0, k)
+    K = np.empty((m, k))
+    v = v0 / np.linalg.norm(v0)
+    for j in range(k):
+        K[:, j] = v
+        v = S @ v
+        v /= np.linalg.norm(v)
+    Q, _ = np.linalg.qr(K)
+    proj = np.linalg.eigvalsh(Q.T @ S @ Q)
+    assert abs(r["theta_max"] - proj[-1]) <= 1e-9 * abs(proj[-1]) and abs(r["theta_min"] - proj[0]) <= 1e-9 * abs(proj[-1])
+    for seed, kk in [(5, 12)] + [(sd, q) for sd in (1, 2, 3) for q in (8, 20, 30)]:
+        rr = O.lanczos_upper_bound(A.apply, d, W.counter_gaussian(seed, 0, m, 1)[:, 0], kk)
+        assert rr["theta_max"] <= lam[-1] * (1 + 1e-12)
+        assert np.min(np.abs(lam - rr["theta_max"])) <= rr["beta_k"] * rr["s_k"] * (1 + 1e-9) + 1e-12
+        assert lam[-1] <= 1.01 * rr["upper"] <= 1.01 * rr["upper_loose"]
+        assert rr["upper"] <= 1.1 * lam[-1]                             # and it is tight, not merely valid
+    T = np.diag([2.0, -1.0, 0.5, 3.0, 1.0]) + 0.3 * np.ones((5, 5))
+    full = O.lanczos_upper_bound(lambda V: T @ V, None, np.arange(1.0, 6.0), 5)
+    ev = np.linalg.eigvalsh(T)
+    assert abs(full["theta_max"] - ev[-1]) < 1e-10 and abs(full["theta_min"] - ev[0]) < 1e-10
+
+
+def test_bounds_gershgorin_and_cellwise_are_upper_bounds():
+    """||D^-1 A||_inf >= spectral radius of D^-1 A (Gershgorin / any induced norm) and max_c lam_max(A_c, B_c) >=
+    lam_max(A, B) (mediant inequality), both against a dense eigensolver on the assembled small pencil."""
+    prob = W.fe_problem(3, q=2, seed=4)
+    A, B, Dinv = O.operators_from_workload(prob)
+    m, d = prob["m"], prob["dinv"]
+    Ad, Bd = A.apply(np.eye(m)), B.apply(np.eye(m))
+    s = np.sqrt(d)
+    lam_d = np.linalg.eigvalsh(s[:, None] * Ad * s[None, :])
+    assert O.gershgorin_upper(Ad, d) >= max(abs(lam_d[0]), abs(lam_d[-1]))
+    assert O.gershgorin_upper(np.diag([1.0, -7.0, 3.0])) == 7.0
+    lam_g = sla.eigh(Ad, Bd, eigvals_only=True)
+    cw = O.fe_cellwise_upper(prob["A_cells"], prob["B_cell"])
+    assert lam_g[-1] <= cw <= 1.3 * lam_g[-1]
