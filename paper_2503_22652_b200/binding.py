@@ -216,7 +216,7 @@ class Rchfsi:
         """Call an entry point; on ENOMEM (workspace exhausted, nothing of the caller's changed) add a torch-owned
         segment of the missing size and repeat."""
         import torch
-        while True:
+        for _attempt in range(64):     # an entry point owns a few dozen buffers at most: more retries mean a bug
             st = fn(self.h, *args)
             if st != ENOMEM or not self._grow:
                 return st
@@ -226,6 +226,7 @@ class Rchfsi:
             # small requests share a 1 MiB segment: fewer, larger torch tensors
             self.add_workspace(torch.empty(max(need, 1 << 20), dtype=torch.uint8,
                                            device=torch.device("cuda", torch.cuda.current_device())))
+        return ENOMEM
 
     def _raise(self, st):
         raise RchfsiError(st, (self.lib.rchfsi_last_error(self.h) or b"").decode())

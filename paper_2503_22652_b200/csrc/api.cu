@@ -243,7 +243,7 @@ size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B
   if (uses & (RCHFSI_USE_RAYLEIGH_RITZ | RCHFSI_USE_SOLVE)) {
     total += (B ? 3 : 2) * al(el * 8);                                                        // A Y, (B Y), rotation target
     total += 2 * al(8 * N * N) + 2 * al(8 * N) + al(16 * N) + al(4);                          // Gram matrices, Ritz values, residuals
-    total += al(8 * (2 * N * N + 8 * N + 64) + (size_t)1 << 20);                              // dsygvd workspace (cuSOLVER query at run time)
+    total += al(8 * (3 * N * N + 16 * N + 64) + ((size_t)8 << 20));                              // dsygvd workspace (cuSOLVER query at run time)
     if (fe) total += fe_rr_scratch_bytes(*A, block_N, A->n_cells);
   }
   if (uses & RCHFSI_USE_SOLVE) total += al(el * 8);                                           // residual block of the solve

@@ -137,7 +137,7 @@ struct rchfsi_ctx {
   float *Gsolve32 = nullptr;                               // [m][N] FP32 residual block of rchfsi_solve (chunked mode)
   double *feg_W = nullptr, *feg_T = nullptr, *feg_A = nullptr;  // fe_rr.cu scratch: gathered operand, product, FP64 cell batch
   const double **feg_ptrs = nullptr;                        // [3][feg_ptr_cap] pointer arrays of the batched GEMM
-  size_t feg_w_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0; int32_t feg_N = 0;
+  size_t feg_w_bytes = 0, feg_W_bytes = 0, feg_T_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0; int32_t feg_N = 0;
   double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;

@@ -126,9 +126,11 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   const int64_t cap = fe_rr_cells_per_batch(op, Nw, max_color);
   const size_t need_w = sizeof(double) * (size_t)cap * nl * Nw;
   h->feg_N = Nw;
+  // every buffer has its own guard: a call that ran out of workspace is repeated after the caller added a segment
+  // (rchfsi_add_workspace) and must not allocate again what it already has
   if (h->feg_w_bytes < need_w) {
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_W, need_w));
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_T, need_w));
+    if (h->feg_W_bytes < need_w) { RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_W, need_w)); h->feg_W_bytes = need_w; }
+    if (h->feg_T_bytes < need_w) { RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_T, need_w)); h->feg_T_bytes = need_w; }
     h->feg_w_bytes = need_w;
   }
   if (conv && h->feg_a_cells < cap) {

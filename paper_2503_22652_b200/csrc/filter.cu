@@ -245,20 +245,18 @@ rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host
   const int32_t w = host_chunk_width(h);
   const int nchunks = (int)cdiv(N, w);
   const int nsets = std::min<int>(rchfsi_ctx::HOST_SETS, nchunks);
-  if (h->host_chunk != w) {
-    if (h->host_chunk != 0) { h->err = "rchfsi_filter_host: staging width changed"; return RCHFSI_EINVAL; }
-    for (int i = 0; i < nsets; ++i) {
-      RCHFSI_TRY(dev_alloc(h, (void **)&h->hX[i], sizeof(double) * (size_t)m * w));
-      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_g[i], cudaEventDisableTiming));
-      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_xin[i], cudaEventDisableTiming));
-      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
-      RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_free[i], cudaEventDisableTiming));
-    }
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->hritz, sizeof(double) * N));
-    RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
-    RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
-    h->host_chunk = w;
+  // (each buffer, event and stream has its own guard: the call may be repeated after the caller added workspace)
+  for (int i = 0; i < nsets; ++i) {
+    if (!h->hX[i]) RCHFSI_TRY(dev_alloc(h, (void **)&h->hX[i], sizeof(double) * (size_t)m * w));
+    if (!h->ev_g[i]) RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_g[i], cudaEventDisableTiming));
+    if (!h->ev_xin[i]) RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_xin[i], cudaEventDisableTiming));
+    if (!h->ev_done[i]) RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+    if (!h->ev_free[i]) RCHFSI_CUDA_CHECK(h, cudaEventCreateWithFlags(&h->ev_free[i], cudaEventDisableTiming));
   }
+  if (!h->hritz) RCHFSI_TRY(dev_alloc(h, (void **)&h->hritz, sizeof(double) * N));
+  if (!h->in_stream) RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking));
+  if (!h->out_stream) RCHFSI_CUDA_CHECK(h, cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking));
+  h->host_chunk = w;
   if (G_host)
     for (int i = 0; i < nsets; ++i)
       if (!h->hG[i]) RCHFSI_TRY(dev_alloc(h, &h->hG[i], gb * (size_t)m * w));

@@ -210,7 +210,7 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
 // FP64 row panel (about 6 GB + 3 GB at config 5 instead of 3 x 58.5 GB).
 bool rr_wants_chunked(rchfsi_ctx *h) {
   if (h->knobs.rr_chunked >= 0) return h->knobs.rr_chunked != 0;               // test / tuning knob
-  if (h->rrc1) return true;                                                    // decided earlier for this handle
+  if (h->rr_cw > 0) return true;                                               // decided earlier for this handle
   if (h->rr1) return false;                                                    // full workspace already there
   size_t free_b = 0, total_b = 0;
   if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return false;
@@ -224,7 +224,7 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   const int64_t m = h->m;
   const int32_t N = h->N;
   cudaStream_t st = h->stream;
-  if (!h->rrc1) {
+  if (h->rr_cw == 0) {
     // two [m][cw] FP64 chunks: 6 GB, or up to a third of the free memory when there is more (wider chunks make the
     // batched FE applies and the Gram GEMMs more efficient)
     size_t free_b = 0, total_b = 0;
@@ -236,10 +236,11 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     rp = std::max<int64_t>(256, std::min<int64_t>(m, rp));
     h->rr_cw = (int32_t)cw;
     h->rr_rp = rp;
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)m * cw));
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc2, sizeof(double) * (size_t)m * cw));
-    RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)rp * N));
   }
+  // (each buffer has its own guard: the call may be repeated after the caller added workspace)
+  if (!h->rrc1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)m * h->rr_cw));
+  if (!h->rrc2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc2, sizeof(double) * (size_t)m * h->rr_cw));
+  if (!h->rrp) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)h->rr_rp * N));
   const int32_t cw = h->rr_cw;
   h->feg_N = std::max(h->feg_N, cw);    // FE apply scratch sized once for the chunk width
   const double one = 1.0, zero = 0.0;
