@@ -186,6 +186,41 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
                             const double *G, int32_t degree, double lam_min, double lam_T,
                             double lam_max);
 
+/* The same filter in three pieces, for callers that must act between the recurrence steps (the row-sharded
+ * multi-GPU filter below): rchfsi_filter == rchfsi_filter_begin; (degree - 1) x rchfsi_filter_step; rchfsi_filter_end.
+ *  begin  validates, computes the scalars and the Lambda_k table, sets R_X = 0, R_Y = (sigma_1/e) G;
+ *  step   one pass of the loop body: the fused operator + recurrence step, then swap(R_X, R_Y);
+ *  end    the last line of Algorithm 3, X <- D^-1 R_Y + X Lambda_Y.  EINVAL while steps are left.
+ * rchfsi_filter_steps_left: steps still to run (0 when no filter is in progress). */
+rchfsi_status rchfsi_filter_begin(rchfsi_handle h, int32_t method, double *X, const double *ritz, const double *G,
+                                  int32_t degree, double lam_min, double lam_T, double lam_max);
+rchfsi_status rchfsi_filter_step(rchfsi_handle h);
+rchfsi_status rchfsi_filter_end(rchfsi_handle h);
+int32_t rchfsi_filter_steps_left(rchfsi_handle h);
+
+/* Row-sharded filter: interface exchange ("nearest-neighbour MPI communication ... in BF16 precision; we
+ * term this method TF32B"; "reducing inter-node message sizes by a factor of 4").  Each rank (one process
+ * per GPU) creates its handle on a SLAB of the operator -- the cells it owns and every row they touch -- so the rows
+ * between two slabs exist on both ranks.  A local rchfsi_filter_step leaves on such a row only this rank's share of the
+ * product: R_new = base + a T_r with base = b R_Y + c' R_X + a G Lambda_Y equal on both ranks.  Per step:
+ *   rchfsi_interface_save(rows)              BEFORE the step: keeps the R_X rows the step will overwrite;
+ *   rchfsi_filter_step
+ *   rchfsi_interface_pack(rows, wire, send)  send[i][j] = wire(R_new - base), i over `rows`, j < N ([n_rows][N], wire type);
+ *   -- the caller swaps `send` with the neighbour rank (NCCL send/recv, torch.distributed) --
+ *   rchfsi_interface_apply(rows, wire, own = send, nbr = received)
+ *                                            R_new = base + (own + nbr), both in wire precision, so the two replicas
+ *                                            of a row stay bit-identical; refreshes the operand shadow of the rows.
+ *  rows       device int32[n_rows]: local row indices of ALL interface rows of this rank (a middle rank: both planes;
+ *             the caller sends / receives the two halves of the buffers to / from its two neighbours).
+ *  wire_prec  RCHFSI_FP64, RCHFSI_FP32 or RCHFSI_BF16: the precision on the wire.  With BF16 the interface rows see an
+ *             O(2^-9) relative error in their share of the product: an inexact matvec (Thm 3.4).
+ * METHOD_RCHFSI with G given only (Algorithm 3 has no operator apply outside the loop).  Asynchronous.
+ * Errors: EINVAL (no filter in progress, bad rows / wire), ENOMEM (workspace), ECUDA. */
+rchfsi_status rchfsi_interface_save(rchfsi_handle h, const int32_t *rows, int32_t n_rows);
+rchfsi_status rchfsi_interface_pack(rchfsi_handle h, const int32_t *rows, int32_t n_rows, int32_t wire_prec, void *send_buf);
+rchfsi_status rchfsi_interface_apply(rchfsi_handle h, const int32_t *rows, int32_t n_rows, int32_t wire_prec,
+                                     const void *own_buf, const void *nbr_buf);
+
 /* Same call with HOST buffers: copies X, ritz (and G if non-NULL) to device scratch,
  * runs rchfsi_filter, copies Y_p back into X_host, synchronises.  G_host holds FP64 values,
  * or FP32 values when the handle was created with g_input_f32. */

@@ -55,6 +55,14 @@ SYMBOLS = {
     "rchfsi_workspace_used": (C.c_size_t, [C.c_void_p]),
     "rchfsi_filter": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                 C.c_double, C.c_double, C.c_double]),
+    "rchfsi_filter_begin": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                      C.c_double, C.c_double, C.c_double]),
+    "rchfsi_filter_step": (C.c_int, [C.c_void_p]),
+    "rchfsi_filter_end": (C.c_int, [C.c_void_p]),
+    "rchfsi_filter_steps_left": (C.c_int32, [C.c_void_p]),
+    "rchfsi_interface_save": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32]),
+    "rchfsi_interface_pack": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]),
+    "rchfsi_interface_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]),
     "rchfsi_filter_host": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                      C.c_double, C.c_double, C.c_double]),
     "rchfsi_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -273,6 +281,41 @@ class Rchfsi:
         if st != OK:
             self._raise(st)
         return X
+
+    # ---- step-wise filter and interface exchange (row-sharded multi-GPU filter; see sharding.py)
+    def filter_begin(self, method, X, ritz, G, degree, lam_min, lam_T, lam_max):
+        self._block(X, "X")
+        st = self._call(self.lib.rchfsi_filter_begin, method, _ptr(X), _ptr(ritz), _ptr(G), degree, lam_min, lam_T, lam_max)
+        if st != OK:
+            self._raise(st)
+
+    def filter_step(self):
+        st = self._call(self.lib.rchfsi_filter_step)
+        if st != OK:
+            self._raise(st)
+
+    def filter_end(self):
+        st = self._call(self.lib.rchfsi_filter_end)
+        if st != OK:
+            self._raise(st)
+
+    def filter_steps_left(self):
+        return int(self.lib.rchfsi_filter_steps_left(self.h))
+
+    def interface_save(self, rows):
+        st = self._call(self.lib.rchfsi_interface_save, _ptr(rows), rows.numel())
+        if st != OK:
+            self._raise(st)
+
+    def interface_pack(self, rows, wire, send):
+        st = self._call(self.lib.rchfsi_interface_pack, _ptr(rows), rows.numel(), PREC[wire], _ptr(send))
+        if st != OK:
+            self._raise(st)
+
+    def interface_apply(self, rows, wire, own, nbr):
+        st = self._call(self.lib.rchfsi_interface_apply, _ptr(rows), rows.numel(), PREC[wire], _ptr(own), _ptr(nbr))
+        if st != OK:
+            self._raise(st)
 
     def filter_host(self, method, X_host, ritz_host, G_host, degree, lam_min, lam_T, lam_max):
         """rchfsi_filter_host: numpy / CPU-tensor buffers (float64, C-contiguous); X_host is

@@ -78,6 +78,23 @@ struct Plan {
 struct Knobs;
 Plan make_plan(const rchfsi_operator &A, int32_t N, const rchfsi_options &opt, const Knobs &kn);
 
+// State of a filter call between rchfsi_filter_begin and rchfsi_filter_end (rchfsi_filter runs the three in one go;
+// the step-wise entry points exist so that a row-sharded caller can exchange interface rows between the steps)
+struct FilterRun {
+  bool active = false;
+  bool chfsi = false, gf32 = false;
+  Plan pl{};
+  double *X = nullptr;
+  int32_t degree = 0, k = 0;            // k = index of the NEXT step to run (2 .. degree)
+  double e = 0, c = 0, sigma1 = 0, gamma = 0, sigma = 0;
+  void *RX = nullptr, *RY = nullptr, *Wcur = nullptr, *Wnext = nullptr;
+  const void *Gst = nullptr;
+  bool g_lib = false;                   // Gst is the library's copy (library layout); else the caller's row-major block
+  uint64_t apply_index = 0;
+  StepCoef last{};                      // coefficients of the step that ran last
+  const double *last_LY = nullptr;      // its Lambda_Y row
+};
+
 // A piece of caller-provided device memory the handle carves its buffers from (rchfsi_add_workspace)
 struct WorkspaceSegment {
   char *base;
@@ -158,6 +175,11 @@ struct rchfsi_ctx {
 
   // rchfsi_estimate_bounds scratch (bounds.cu)
   double *bnd_buf = nullptr, *bnd_cell = nullptr, *bnd_work = nullptr;
+
+  rchfsi::FilterRun run;
+  // interface exchange of a row-sharded filter (interface.cu): saved old R_X rows and the recomputed base term
+  void *if_old = nullptr, *if_base = nullptr;
+  size_t if_cap = 0, if_old_cap = 0, if_base_cap = 0;   // rows x N_cap elements the buffers hold
 
   // instrumentation
   cudaEvent_t ev_step0 = nullptr, ev_step1 = nullptr;

@@ -91,11 +91,13 @@ rchfsi_status do_step(rchfsi_ctx *h, const Plan &pl, bool chfsi, const StepCoef 
 }  // namespace
 
 // G_arg points to FP64 values, or to FP32 values when g_is_f32 (caller's g_input_f32 option, or the FP32
-// residual block rchfsi_solve keeps in its memory-light mode)
-static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, const double *ritz, const void *G_arg,
-                                 bool g_is_f32, int32_t degree, double lam_min, double lam_T, double lam_max) {
+// residual block rchfsi_solve keeps in its memory-light mode).  Validation, workspace, scalars, Lambda table and the
+// initial blocks: everything of Alg. 2 / Alg. 3 before the loop.
+static rchfsi_status filter_begin(rchfsi_handle h, int32_t method, double *X, const double *ritz, const void *G_arg,
+                                  bool g_is_f32, int32_t degree, double lam_min, double lam_T, double lam_max) {
   const double *G = reinterpret_cast<const double *>(G_arg);
   if (!h) return RCHFSI_EINVAL;
+  h->run.active = false;
   if (!X || (reinterpret_cast<uintptr_t>(X) & 15u)) { h->err = "rchfsi_filter: X null or misaligned"; return RCHFSI_EINVAL; }
   if (method != RCHFSI_METHOD_CHFSI && method != RCHFSI_METHOD_RCHFSI) { h->err = "rchfsi_filter: unknown method"; return RCHFSI_EINVAL; }
   if (method == RCHFSI_METHOD_RCHFSI && !ritz) { h->err = "rchfsi_filter: ritz is required for R-ChFSI"; return RCHFSI_EINVAL; }
@@ -110,36 +112,41 @@ static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, con
     h->err = "rchfsi_filter: need lam_min < lam_T < lam_max";
     return RCHFSI_EINVAL;
   }
-  const bool chfsi = (method == RCHFSI_METHOD_CHFSI);
-  const Plan pl = make_plan(h);
+  FilterRun &r = h->run;
+  r = FilterRun{};
+  r.chfsi = (method == RCHFSI_METHOD_CHFSI);
+  r.pl = make_plan(h);
+  const Plan &pl = r.pl;
   const int64_t m = h->m;
   const int32_t N = h->N;
   const size_t el = (size_t)m * N;
   cudaStream_t st = h->stream;
   // FP32 residual block from the caller (g_input_f32): used in place, never copied (config 5 memory plan)
-  const bool gf32 = !chfsi && g_is_f32;
-  if (gf32 && (!G || pl.store != RCHFSI_FP32)) {
+  r.gf32 = !r.chfsi && g_is_f32;
+  if (r.gf32 && (!G || pl.store != RCHFSI_FP32)) {
     h->err = "rchfsi_filter: g_input_f32 needs a non-NULL G and store_prec FP32";
     return RCHFSI_EINVAL;
   }
-  const bool need_gs = !chfsi && !gf32 && (pl.store != RCHFSI_FP64 || pl.panel);
+  const bool need_gs = !r.chfsi && !r.gf32 && (pl.store != RCHFSI_FP64 || pl.panel);
   const int64_t pm = pl.panel ? m : 0;
   const size_t el_lib = pl.panel ? (size_t)m * (size_t)cdiv(N, 128) * 128 : el;
   RCHFSI_TRY(ensure_filter_workspace(h, pl, degree, need_gs));
 
   // first line of Alg. 2 / Alg. 3
-  const double e = (lam_max - lam_T) / 2.0;
-  const double c = (lam_max + lam_T) / 2.0;
-  const double sigma1 = e / (lam_min - c);
-  const double gamma = 2.0 / sigma1;
-  double sigma = sigma1;
+  r.e = (lam_max - lam_T) / 2.0;
+  r.c = (lam_max + lam_T) / 2.0;
+  r.sigma1 = r.e / (lam_min - r.c);
+  r.gamma = 2.0 / r.sigma1;
+  r.sigma = r.sigma1;
+  r.X = X;
+  r.degree = degree;
+  r.RX = h->RX;
+  r.RY = h->RY;
+  r.Wcur = pl.shadow ? h->Wa : nullptr;
+  r.Wnext = pl.shadow ? (pl.shadow_inplace ? h->Wa : h->Wb) : nullptr;
+  const double e = r.e, c = r.c, sigma1 = r.sigma1;
 
-  void *RX = h->RX, *RY = h->RY;
-  void *Wcur = pl.shadow ? h->Wa : nullptr, *Wnext = pl.shadow ? (pl.shadow_inplace ? h->Wa : h->Wb) : nullptr;
-  const void *Gst = nullptr;
-  uint64_t apply_index = 0;
-
-  if (!chfsi) {
+  if (!r.chfsi) {
     // G = A X - B X Lambda with the exact operators (reading S5) when the caller has none
     if (!G) {
       const size_t el_cap = (size_t)m * h->N_cap;
@@ -155,60 +162,86 @@ static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, con
       G = h->Gtmp;
     }
     RCHFSI_TRY(lambda_table(h, ritz, N, degree, e, c, sigma1, h->lam_table));
-    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RX, 0, el_lib * prec_bytes(pl.store), st));       // R_X <- 0
-    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, RY, Wcur, m, N, pm,
-                             gf32 ? RCHFSI_FP32 : RCHFSI_FP64));                          // R_Y <- (sigma_1/e) G
+    RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(r.RX, 0, el_lib * prec_bytes(pl.store), st));     // R_X <- 0
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, sigma1 / e, G, r.RY, r.Wcur, m, N, pm,
+                             r.gf32 ? RCHFSI_FP32 : RCHFSI_FP64));                        // R_Y <- (sigma_1/e) G
     if (need_gs) {
       RCHFSI_TRY(scale_convert(h, pl.store, 0, 1.0, G, h->Gs, nullptr, m, N, pm));
-      Gst = h->Gs;
+      r.Gst = h->Gs;
+      r.g_lib = true;
     } else {
-      Gst = G;
+      r.Gst = G;
     }
   } else {
     // Alg. 2: X_k = X, Y = (sigma_1/e)(D^-1 A (x) X - c X)
-    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, 1.0, X, RX, Wcur, m, N, pm));
-    const void *W0 = pl.shadow ? Wcur : RX;
+    RCHFSI_TRY(scale_convert(h, pl.store, pl.operand, 1.0, X, r.RX, r.Wcur, m, N, pm));
+    const void *W0 = pl.shadow ? r.Wcur : r.RX;
     if (pl.fused) {
       // first step through the fused kernels: RY <- a T + b X with a = sigma_1/e, b = -a c, c' = 0
-      RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(RY, 0, el_lib * prec_bytes(pl.store), st));
+      RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(r.RY, 0, el_lib * prec_bytes(pl.store), st));
       StepCoef k0{sigma1 / e, -(sigma1 / e) * c, 0.0};
-      RCHFSI_TRY(do_step(h, pl, true, k0, W0, RX, RY, nullptr, nullptr, Wnext, apply_index++));
+      RCHFSI_TRY(do_step(h, pl, true, k0, W0, r.RX, r.RY, nullptr, nullptr, r.Wnext, r.apply_index++));
     } else {
       if (pl.tprec == RCHFSI_FP64)
         RCHFSI_TRY(op_apply_simt<double>(h, h->A.d, nullptr, (const double *)W0, (double *)h->T, N));
       else
         RCHFSI_TRY(op_apply_simt<float>(h, h->A.d, nullptr, (const float *)W0, (float *)h->T, N));
       if (h->opt.noise_eps > 0)
-        RCHFSI_TRY(add_column_noise(h, pl.tprec, h->T, m, N, h->opt.noise_eps, h->opt.noise_seed, apply_index, h->colnorm));
-      apply_index++;
-      RCHFSI_TRY(chfsi_first(h, pl.store, pl.tprec, pl.operand, sigma1 / e, c, h->T, h->dinv, X, RY, Wnext, m, N));
+        RCHFSI_TRY(add_column_noise(h, pl.tprec, h->T, m, N, h->opt.noise_eps, h->opt.noise_seed, r.apply_index, h->colnorm));
+      r.apply_index++;
+      RCHFSI_TRY(chfsi_first(h, pl.store, pl.tprec, pl.operand, sigma1 / e, c, h->T, h->dinv, X, r.RY, r.Wnext, m, N));
     }
-    if (pl.shadow) std::swap(Wcur, Wnext);
+    if (pl.shadow) std::swap(r.Wcur, r.Wnext);
   }
+  r.k = 2;
+  r.active = true;
+  return RCHFSI_OK;
+}
 
-  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step0, st));
-  for (int32_t k = 2; k <= degree; ++k) {
-    const double sigma2 = 1.0 / (gamma - sigma);
-    StepCoef kc{2.0 * sigma2 / e, -2.0 * sigma2 * c / e, -sigma * sigma2};
-    const double *LY = chfsi ? nullptr : h->lam_table + (size_t)(k - 1) * N;
-    const void *W = pl.shadow ? Wcur : RY;
-    RCHFSI_TRY(do_step(h, pl, chfsi, kc, W, RY, RX, chfsi ? nullptr : Gst, LY, Wnext, apply_index++, gf32));
-    std::swap(RX, RY);                       // swap(R_X, R_Y)
-    if (pl.shadow) std::swap(Wcur, Wnext);
-    sigma = sigma2;
-  }
-  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step1, st));
-  h->last_steps = degree - 1;
+// One pass of the loop body of Alg. 2 / Alg. 3: the fused operator + recurrence step k, then swap(R_X, R_Y).
+static rchfsi_status filter_step(rchfsi_handle h) {
+  FilterRun &r = h->run;
+  if (!r.active || r.k > r.degree) { h->err = "rchfsi_filter_step: no step left (call rchfsi_filter_begin first)"; return RCHFSI_EINVAL; }
+  const int32_t N = h->N;
+  const double sigma2 = 1.0 / (r.gamma - r.sigma);
+  StepCoef kc{2.0 * sigma2 / r.e, -2.0 * sigma2 * r.c / r.e, -r.sigma * sigma2};
+  const double *LY = r.chfsi ? nullptr : h->lam_table + (size_t)(r.k - 1) * N;
+  const void *W = r.pl.shadow ? r.Wcur : r.RY;
+  RCHFSI_TRY(do_step(h, r.pl, r.chfsi, kc, W, r.RY, r.RX, r.chfsi ? nullptr : r.Gst, LY, r.Wnext, r.apply_index++, r.gf32));
+  std::swap(r.RX, r.RY);                       // swap(R_X, R_Y)
+  if (r.pl.shadow) std::swap(r.Wcur, r.Wnext);
+  r.sigma = sigma2;
+  r.last = kc;
+  r.last_LY = LY;
+  r.k++;
+  return RCHFSI_OK;
+}
 
+// Last line of Alg. 3, Y_p = D^-1 R_Y + X Lambda_Y; Alg. 2: the block itself.
+static rchfsi_status filter_end(rchfsi_handle h) {
+  FilterRun &r = h->run;
+  if (!r.active || r.k <= r.degree) { h->err = "rchfsi_filter_end: steps are left (or no filter was begun)"; return RCHFSI_EINVAL; }
+  const int64_t m = h->m;
+  const int32_t N = h->N;
+  const int64_t pm = r.pl.panel ? m : 0;
+  r.active = false;
   if (h->x_pending) {   // rchfsi_filter_host: X is still arriving on the copy stream
     h->x_pending = false;
-    RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(st, h->ev_x, 0));
+    RCHFSI_CUDA_CHECK(h, cudaStreamWaitEvent(h->stream, h->ev_x, 0));
   }
-  if (!chfsi)   // Y_p = D^-1 R_Y + X Lambda_Y
-    RCHFSI_TRY(finish_block(h, pl.store, RY, h->dinv, h->lam_table + (size_t)degree * N, X, m, N, pm));
-  else
-    RCHFSI_TRY(finish_block(h, pl.store, RY, nullptr, nullptr, X, m, N, pm));
-  return RCHFSI_OK;
+  if (!r.chfsi)
+    return finish_block(h, r.pl.store, r.RY, h->dinv, h->lam_table + (size_t)r.degree * N, r.X, m, N, pm);
+  return finish_block(h, r.pl.store, r.RY, nullptr, nullptr, r.X, m, N, pm);
+}
+
+static rchfsi_status filter_impl(rchfsi_handle h, int32_t method, double *X, const double *ritz, const void *G_arg,
+                                 bool g_is_f32, int32_t degree, double lam_min, double lam_T, double lam_max) {
+  RCHFSI_TRY(filter_begin(h, method, X, ritz, G_arg, g_is_f32, degree, lam_min, lam_T, lam_max));
+  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step0, h->stream));
+  for (int32_t k = 2; k <= degree; ++k) RCHFSI_TRY(filter_step(h));
+  RCHFSI_CUDA_CHECK(h, cudaEventRecord(h->ev_step1, h->stream));
+  h->last_steps = degree - 1;
+  return filter_end(h);
 }
 
 extern "C" {
@@ -218,6 +251,15 @@ rchfsi_status rchfsi_filter(rchfsi_handle h, int32_t method, double *X, const do
   if (!h) return RCHFSI_EINVAL;
   return filter_impl(h, method, X, ritz, G, h->opt.g_input_f32 != 0, degree, lam_min, lam_T, lam_max);
 }
+
+rchfsi_status rchfsi_filter_begin(rchfsi_handle h, int32_t method, double *X, const double *ritz, const double *G,
+                                  int32_t degree, double lam_min, double lam_T, double lam_max) {
+  if (!h) return RCHFSI_EINVAL;
+  return filter_begin(h, method, X, ritz, G, h->opt.g_input_f32 != 0, degree, lam_min, lam_T, lam_max);
+}
+rchfsi_status rchfsi_filter_step(rchfsi_handle h) { return h ? filter_step(h) : RCHFSI_EINVAL; }
+rchfsi_status rchfsi_filter_end(rchfsi_handle h) { return h ? filter_end(h) : RCHFSI_EINVAL; }
+int32_t rchfsi_filter_steps_left(rchfsi_handle h) { return (h && h->run.active) ? h->run.degree - h->run.k + 1 : 0; }
 
 // Column-chunked host pipeline.  The columns of the block are independent through the whole filter (Alg. 3 touches
 // column j only through eps_j and Lambda_k[j]), so the block is cut into column chunks and chunk
