@@ -14,6 +14,7 @@ so that it can be checked against PAPER.md by eye:
   filter_chfsi        Algorithm 2 / eq. (2), eq. (7)
   filter_rchfsi       Algorithm 3 / eqs. (11)-(13)
   rayleigh_ritz       Step 2-3 of Algorithm 1
+                      (Y^dagger = conjugate transpose: complex Hermitian pencils of PAPER.md:373-401 included)
   residual_norms      r_j = ||A x_j - eps_j B x_j||_2
   solve               Algorithm 1 (do-while reading S1)
   tan_max_angle       Definition 2.1
@@ -41,7 +42,8 @@ import scipy.linalg as sla
 # --------------------------------------------------------------------------- operators
 class DenseOperator:
     def __init__(self, A):
-        self.A = np.asarray(A, dtype=np.float64)
+        A = np.asarray(A)
+        self.A = A.astype(np.complex128 if np.iscomplexobj(A) else np.float64)
         self.m = self.A.shape[0]
 
     def apply(self, V):
@@ -239,14 +241,16 @@ def rayleigh_ritz(apply_A, apply_B, Y, normalize_columns=True):
     solve (Y^T A Y) E = (Y^T B Y) E Lambda with E^T (Y^T B Y) E = I, eigenvalues
     ascending, X = Y E.  Columns of Y are first scaled to unit 2-norm (reading S6;
     it changes neither the subspace nor the Ritz pairs).  Returns (ritz, X, AX, BX)."""
+    # "Y^dagger" of PAPER.md:55 is the conjugate transpose: complex Hermitian problems (PAPER.md:373-401) go through
+    # the same lines; for real blocks conj() is the identity
     if normalize_columns:
-        Y = Y / np.sqrt(np.sum(Y * Y, axis=0))[None, :]
+        Y = Y / np.sqrt(np.sum(np.abs(Y) ** 2, axis=0))[None, :]
     AY = apply_A(Y)
     BY = apply_B(Y)
-    Ha = Y.T @ AY
-    Hb = Y.T @ BY
-    Ha = 0.5 * (Ha + Ha.T)
-    Hb = 0.5 * (Hb + Hb.T)
+    Ha = Y.conj().T @ AY
+    Hb = Y.conj().T @ BY
+    Ha = 0.5 * (Ha + Ha.conj().T)
+    Hb = 0.5 * (Hb + Hb.conj().T)
     ritz, E = sla.eigh(Ha, Hb)             # LAPACK dsygv-type: E^T Hb E = I, ascending
     return ritz, Y @ E, AY @ E, BY @ E
 
@@ -259,7 +263,7 @@ def residual_block(AX, BX, ritz):
 def residual_norms(AX, BX, ritz):
     """r_j = ||A x_j - eps_j B x_j||_2, absolute (reading S8)."""
     G = residual_block(AX, BX, ritz)
-    return np.sqrt(np.sum(G * G, axis=0))
+    return np.sqrt(np.sum(np.abs(G) ** 2, axis=0))
 
 
 # --------------------------------------------------------------------------- Algorithm 1

@@ -268,7 +268,7 @@ static int32_t host_chunk_width(const rchfsi_ctx *h) {
   const int32_t N = h->N_cap;
   if (h->knobs.host_chunk >= 128) return std::min<int32_t>((int32_t)cdiv(h->knobs.host_chunk, 128) * 128, N);   // test knob
   const double blk = 8.0 * (double)h->m * N;
-  if (blk < 256e6 || N < 512) return N;               // small blocks: one chunk (the X upload still overlaps the steps)
+  if (blk < 256e6 || N < 256) return N;               // small blocks: one chunk (the X upload still overlaps the steps)
   int32_t w = (int32_t)cdiv(cdiv(N, 6), 128) * 128;   // about six chunks, whole 128-column tiles
   return std::min(w, N);
 }
