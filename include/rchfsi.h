@@ -286,6 +286,35 @@ rchfsi_status rchfsi_apply(rchfsi_handle h, int32_t which, const double *V, doub
 int64_t rchfsi_launch_count(rchfsi_handle h);
 rchfsi_status rchfsi_last_filter_step_ms(rchfsi_handle h, float *ms_total_out, int32_t *steps_out);
 
+/* ---------------------------------------------------------------------------------------------
+ * Allocation-free entry point for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  No handle, no workspace: its scratch is a file-scope __device__ array of
+ * RCHFSI_STATIC_SCRATCH_BYTES (148 slots x RCHFSI_STATIC_MAX_N partial sums + a 256-byte header) that every GPU
+ * which loads the library holds until the process exits.
+ *
+ * rchfsi_residual_static: G = AX - BX diag(ritz) (the residual block of Algorithm 3) and
+ * r_j = ||A x_j - ritz_j B x_j||_2, FP64, on the CURRENT device.
+ *  AX, BX       device [m][N] row-major FP64: A X and B X (pass X itself as BX for a standard problem).
+ *  ritz         device [N].
+ *  G_out        device [m][N] or NULL, not aliasing an input.  resnorm_out device [N] or NULL; not both NULL.
+ *  stream       cudaStream_t (NULL = the default stream).  Asynchronous: one kernel launch, nothing else.
+ * N > RCHFSI_STATIC_MAX_N, non-positive sizes or NULL inputs return RCHFSI_EINVAL with outputs untouched
+ * (rchfsi_static_last_error, per host thread).  Calls no cudaMalloc / cudaFree / allocating library routine.
+ * The partial sums are added in a fixed order, so r_j is bitwise reproducible (the atomicAdd reduction inside
+ * rchfsi_rayleigh_ritz is not).  ALL calls on one device share the scratch array, which keeps the last call's
+ * contents; the kernel re-arms its ticket counter itself.  Two calls that overlap on the GPU (different streams, or
+ * different host threads) race on it: serialise them.  A call whose kernel was aborted leaves the counter undefined.
+ *
+ * rchfsi_static_setup: takes the array's device address (cudaGetSymbolAddress) and clears the counter for the CURRENT
+ * device, once; rchfsi_residual_static does it lazily on first use, but a caller that captures a CUDA graph must call
+ * it before the capture starts (the set-up synchronises). */
+#define RCHFSI_STATIC_MAX_N 4096
+#define RCHFSI_STATIC_SCRATCH_BYTES 4849920
+rchfsi_status rchfsi_static_setup(void);
+rchfsi_status rchfsi_residual_static(const double *AX, const double *BX, const double *ritz, int64_t m, int32_t N,
+                                     double *G_out, double *resnorm_out, void *stream);
+const char *rchfsi_static_last_error(void);
+
 /* Library / build identification, e.g. "rchfsi 0.1 sm_100a". */
 const char *rchfsi_version(void);
 

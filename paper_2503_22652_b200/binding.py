@@ -73,7 +73,12 @@ SYMBOLS = {
     "rchfsi_apply": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
     "rchfsi_launch_count": (C.c_int64, [C.c_void_p]),
     "rchfsi_last_filter_step_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]),
+    "rchfsi_static_setup": (C.c_int, []),
+    "rchfsi_residual_static": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p,
+                                         C.c_void_p, C.c_void_p]),
+    "rchfsi_static_last_error": (C.c_char_p, []),
 }
+STATIC_MAX_N = 4096          # RCHFSI_STATIC_MAX_N
 
 _lib = None
 
@@ -401,3 +406,34 @@ class Rchfsi:
         if st != OK:
             self._raise(st)
         return ms.value, n.value
+
+
+# ------------------------------------------------------------------------- allocation-free entry point
+def static_setup():
+    """rchfsi_static_setup on the current device (needed before a CUDA graph capture; otherwise lazy)."""
+    lib = load_library()
+    st = lib.rchfsi_static_setup()
+    if st != OK:
+        raise RchfsiError(st, (lib.rchfsi_static_last_error() or b"").decode())
+
+
+def residual_static(AX, BX, ritz, G_out=None, resnorm_out=None, stream=None):
+    """rchfsi_residual_static: G_out = AX - BX diag(ritz), resnorm_out[j] = ||G_j||_2, written into the CALLER's
+    tensors ([m][N] / [N], FP64, contiguous, CUDA); the library allocates nothing (static device scratch, N <= 4096).
+    Marshalling only: no tensor is created here."""
+    import torch
+    lib = load_library()
+    _check_dev(AX, torch.float64, "AX")
+    _check_dev(BX, torch.float64, "BX")
+    _check_dev(ritz, torch.float64, "ritz")
+    if AX.dim() != 2 or BX.shape != AX.shape or ritz.numel() != AX.shape[1]:
+        raise ValueError("AX, BX must be [m][N] and ritz [N]")
+    if G_out is not None and (_check_dev(G_out, torch.float64, "G_out").shape != AX.shape):
+        raise ValueError("G_out must be [m][N]")
+    if resnorm_out is not None and _check_dev(resnorm_out, torch.float64, "resnorm_out").numel() != AX.shape[1]:
+        raise ValueError("resnorm_out must be [N]")
+    s = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    st = lib.rchfsi_residual_static(_ptr(AX), _ptr(BX), _ptr(ritz), AX.shape[0], AX.shape[1], _ptr(G_out),
+                                    _ptr(resnorm_out), C.c_void_p(s))
+    if st != OK:
+        raise RchfsiError(st, (lib.rchfsi_static_last_error() or b"").decode())
