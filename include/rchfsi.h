@@ -240,6 +240,14 @@ rchfsi_status rchfsi_filter_host(rchfsi_handle h, int32_t method, double *X_host
 rchfsi_status rchfsi_rayleigh_ritz(rchfsi_handle h, double *Y_in_X_out, double *ritz_out,
                                    double *G_out, double *resnorm_out);
 
+/* The subspace rotation of the Rayleigh-Ritz step on its own ("X = Y E"): Y <- Y E in place, FP64.
+ *  Y_in_X_out    device [m][N] row-major.
+ *  E_colmajor    device N x N, column-major (the LAPACK / cuSOLVER eigenvector layout), not aliasing Y.
+ * Same kernel choice as inside rchfsi_rayleigh_ritz: the INT8 tensor-pipe product of rr_i8.cu for large blocks
+ * (error-free digit split of both operands, result within a few FP64 ulps of (row max of Y) x (column max of E) per
+ * element), cuBLAS dgemm otherwise; RCHFSI_RR_SPLIT=0/1 forces the choice.  Asynchronous. */
+rchfsi_status rchfsi_rotate(rchfsi_handle h, double *Y_in_X_out, const double *E_colmajor);
+
 /* Algorithm 1, do-while reading: one Rayleigh-Ritz on the initial guess,
  * then repeat { filter; Rayleigh-Ritz; residual test on the n_wanted lowest pairs }.
  *  X            device [m][N]: in the initial guess, out B-orthonormal Ritz vectors.

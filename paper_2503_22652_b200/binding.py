@@ -66,6 +66,7 @@ SYMBOLS = {
     "rchfsi_filter_host": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                      C.c_double, C.c_double, C.c_double]),
     "rchfsi_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rchfsi_rotate": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rchfsi_solve": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p,
                                C.POINTER(C.c_int32), C.c_void_p]),
@@ -361,6 +362,19 @@ class Rchfsi:
         if st != OK:
             self._raise(st)
         return ritz, Y, G, res
+
+    def rotate(self, Y, E_colmajor):
+        """rchfsi_rotate: Y <- Y E in place; E_colmajor is a contiguous [N][N] CUDA tensor holding E COLUMN-major
+        (i.e. E.T.contiguous() of a row-major E)."""
+        import torch
+        self._block(Y, "Y")
+        _check_dev(E_colmajor, torch.float64, "E")
+        if tuple(E_colmajor.shape) != (self.N, self.N):
+            raise ValueError("E must be [N][N]")
+        st = self._call(self.lib.rchfsi_rotate, _ptr(Y), _ptr(E_colmajor))
+        if st != OK:
+            self._raise(st)
+        return Y
 
     def solve(self, method, X, n_wanted, degree, lam_min, lam_T, lam_max, tol=1e-8, max_iter=50,
               raise_on_not_converged=False):

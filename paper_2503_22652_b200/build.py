@@ -11,7 +11,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librchfsi.so")
 SOURCES = ["api.cu", "filter.cu", "kernels_simt.cu", "elementwise.cu", "rr.cu", "csr_fused.cu",
-           "dense_tc.cu", "fe_tc.cu", "fe_rr.cu", "bounds.cu", "interface.cu", "residual_static.cu"]
+           "dense_tc.cu", "fe_tc.cu", "fe_rr.cu", "rr_i8.cu", "bounds.cu", "interface.cu", "residual_static.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]

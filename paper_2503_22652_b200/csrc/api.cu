@@ -84,6 +84,8 @@ static Knobs read_knobs() {
   k.rr_fe_simt = getenv("RCHFSI_RR_FE_SIMT") != nullptr;
   k.rr_timing = getenv("RCHFSI_RR_TIMING") != nullptr;
   k.rr_split = geti("RCHFSI_RR_SPLIT", -1);
+  k.rr_i8_rows = geti("RCHFSI_RR_I8_ROWS", 0);
+  k.rr_gram_i8 = geti("RCHFSI_RR_GRAM_I8", -1);
   k.host_chunk = geti("RCHFSI_HOST_CHUNK", 0);
 #ifdef RCHFSI_PROBES
   k.tc_debug = geti("RCHFSI_TC_DEBUG", 0);
@@ -245,6 +247,7 @@ size_t rchfsi_workspace_bytes(const rchfsi_operator *A, const rchfsi_operator *B
     total += 2 * al(8 * N * N) + 2 * al(8 * N) + al(16 * N) + al(4);                          // Gram matrices, Ritz values, residuals
     total += al(8 * (3 * N * N + 16 * N + 64) + ((size_t)8 << 20));                              // dsygvd workspace (cuSOLVER query at run time)
     if (fe) total += fe_rr_scratch_bytes(*A, block_N, A->n_cells);
+    total += rr_i8_plan_bytes((int64_t)m, block_N) + al(std::min<size_t>(el * 8, (size_t)3e9 + 8 * N));   // INT8 products (rr_i8.cu), row panel of rchfsi_rotate
   }
   if (uses & RCHFSI_USE_SOLVE) total += al(el * 8);                                           // residual block of the solve
   if (uses & RCHFSI_USE_FILTER_HOST) {
@@ -266,6 +269,16 @@ rchfsi_status rchfsi_apply(rchfsi_handle h, int32_t which, const double *V, doub
     return RCHFSI_OK;
   }
   return op_apply_simt<double>(h, which == 0 ? h->A.d : h->B.d, nullptr, V, out, h->N);
+}
+
+rchfsi_status rchfsi_rotate(rchfsi_handle h, double *Y_in_X_out, const double *E_colmajor) {
+  if (!h) return RCHFSI_EINVAL;
+  if (!Y_in_X_out || !E_colmajor || !aligned16(Y_in_X_out) || !aligned16(E_colmajor)) {
+    h->err = "rchfsi_rotate: null or misaligned argument";
+    return RCHFSI_EINVAL;
+  }
+  if (h->run.active) { h->err = "rchfsi_rotate: a step-wise filter is in progress"; return RCHFSI_EINVAL; }
+  return rotate_in_place(h, Y_in_X_out, E_colmajor);
 }
 
 rchfsi_status rchfsi_rayleigh_ritz(rchfsi_handle h, double *Y_in_X_out, double *ritz_out, double *G_out,

@@ -58,10 +58,16 @@ struct Knobs {
   int rr_chunked = -1;           // RCHFSI_RR_CHUNKED: force the memory-light Rayleigh-Ritz on / off
   bool rr_fe_simt = false;       // RCHFSI_RR_FE_SIMT: FE applies of the Rayleigh-Ritz through the hand-written FP64 kernel
   bool rr_timing = false;        // RCHFSI_RR_TIMING: print phase times of the Rayleigh-Ritz to stderr
-  int rr_split = -1;             // RCHFSI_RR_SPLIT: Gram / rotation products on the tensor pipe (split operands), -1 = automatic
+  int rr_split = -1;             // RCHFSI_RR_SPLIT: rotation X = Y E on the INT8 tensor pipe (rr_i8.cu): 0 off, 1 forced, -1 = automatic
+  int rr_gram_i8 = -1;           // RCHFSI_RR_GRAM_I8: Gram products Y^T (Op Y) on the INT8 tensor pipe: 0 off, 1 forced, -1 = automatic
+  int rr_i8_rows = 0;            // RCHFSI_RR_I8_ROWS: cap on the rows of one digit-plane chunk (tests: forces several chunks)
   int host_chunk = 0;            // RCHFSI_HOST_CHUNK: column-chunk width of rchfsi_filter_host (multiple of 128), 0 = automatic
   int tc_debug = 0;              // RCHFSI_TC_DEBUG (only in -DRCHFSI_PROBES builds)
 };
+
+// rr_i8.cu: a device buffer lent for digit planes, and the planes of the column-slab Gram products
+struct I8Buf { void *ptr; size_t bytes; };
+struct I8GramState { bool active = false; int8_t *yp[7] = {}, *zp[7] = {}; int64_t Rp = 0; int32_t max_w = 0; };
 
 // How rchfsi_filter lays out its blocks for (operator, block width, options): which fused kernel runs, which
 // precision the operand block has, whether an operand shadow exists.  Decided from the descriptor alone so that
@@ -156,6 +162,10 @@ struct rchfsi_ctx {
   const double **feg_ptrs = nullptr;                        // [3][feg_ptr_cap] pointer arrays of the batched GEMM
   size_t feg_w_bytes = 0, feg_W_bytes = 0, feg_T_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0; int32_t feg_N = 0;
   double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
+  void *i8_cols = nullptr, *i8_hpart = nullptr; size_t i8_hpart_bytes = 0;   // rr_i8.cu: column maxima / exponents, K-split partial Gram sums
+  rchfsi::I8GramState i8g;                                  // transposed digit planes of Y of the memory-light Rayleigh-Ritz
+  size_t RX_bytes = 0, RY_bytes = 0, Wa_bytes = 0;        // sizes of the filter's blocks (lent to the Rayleigh-Ritz between filters)
+  void *i8_E = nullptr;                                    // rr_i8.cu: digit planes + exponents of the eigenvector matrix
   double *ritz_dev = nullptr, *res_dev = nullptr;          // [N]
   double *sy_work = nullptr; int sy_lwork = 0; int *sy_info = nullptr;
 
@@ -326,5 +336,20 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
 rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, void *G_out, int g_prec,
                                     double *res_out);
 bool rr_wants_chunked(rchfsi_ctx *h);
+rchfsi_status rotate_in_place(rchfsi_ctx *h, double *Y, const double *E);   // rchfsi_rotate
+
+// ---- rr_i8.cu: rotation X = Y E on the INT8 tensor pipe (error-free digit split of the FP64 operands) ----
+bool rotate_i8_supported(const rchfsi_ctx *h);
+size_t rotate_i8_fixed_bytes(int32_t N);        // digit planes of E, held by the handle
+// Out[r][:] = In[r][:] E for r < rows (E column-major N x N); Out may be In; `scratch` holds one row chunk's planes
+rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const double *E, double *Out, void *scratch,
+                        size_t scratch_bytes);
+// Gram products H = Y^T Z (lower triangle, column-major) with the same digit split, contraction over the rows
+bool gram_i8_supported(const rchfsi_ctx *h);
+size_t rr_i8_plan_bytes(int64_t m, int32_t N);   // digit planes of E, column exponents, K-split partial sums
+rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, const double *BY, double *Ha, double *Hb,
+                           void *scratch, size_t scratch_bytes);
+bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int32_t max_w, rchfsi_status *st);
+rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Z, int64_t ldz, int32_t w, int32_t zc0, double *H);
 
 }  // namespace rchfsi

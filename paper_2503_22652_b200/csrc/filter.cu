@@ -48,11 +48,11 @@ Plan make_plan(const rchfsi_ctx *h) { return rchfsi::make_plan(h->A.d, h->N, h->
 rchfsi_status ensure_filter_workspace(rchfsi_ctx *h, const Plan &pl, int32_t degree, bool need_gs) {
   // sized for the block width of rchfsi_create (N_cap), whatever the active width of this call
   const size_t el = (size_t)h->m * (pl.panel ? (size_t)cdiv(h->N_cap, 128) * 128 : (size_t)h->N_cap);
-  if (!h->RX) RCHFSI_TRY(dev_alloc(h, &h->RX, el * prec_bytes(pl.store)));
-  if (!h->RY) RCHFSI_TRY(dev_alloc(h, &h->RY, el * prec_bytes(pl.store)));
+  if (!h->RX) { RCHFSI_TRY(dev_alloc(h, &h->RX, el * prec_bytes(pl.store))); h->RX_bytes = el * prec_bytes(pl.store); }
+  if (!h->RY) { RCHFSI_TRY(dev_alloc(h, &h->RY, el * prec_bytes(pl.store))); h->RY_bytes = el * prec_bytes(pl.store); }
   if (pl.shadow) {
     const size_t wb = el * (pl.operand == RCHFSI_BF16 ? 2 : 4);
-    if (!h->Wa) RCHFSI_TRY(dev_alloc(h, &h->Wa, wb));
+    if (!h->Wa) { RCHFSI_TRY(dev_alloc(h, &h->Wa, wb)); h->Wa_bytes = wb; }
     if (!pl.shadow_inplace && !h->Wb) RCHFSI_TRY(dev_alloc(h, &h->Wb, wb));
   }
   if (pl.fused == 0 && !h->T) RCHFSI_TRY(dev_alloc(h, &h->T, el * prec_bytes(pl.tprec)));

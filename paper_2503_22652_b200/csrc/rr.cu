@@ -1,7 +1,7 @@
 // Rayleigh-Ritz on a non-orthogonal basis, FP64 throughout.
-// Off the hot path: the Gram and rotation products are plain library
-// GEMMs (cuBLAS dgemm) and the N x N generalized eigenproblem is cuSOLVER dsygvd; the operator
-// applies are this library's FP64 kernels.
+// Off the hot path: the Gram products are plain library GEMMs (cuBLAS dgemm), the rotation
+// X = Y E runs on the INT8 tensor pipe for large blocks (rr_i8.cu, dgemm otherwise), the N x N generalized
+// eigenproblem is cuSOLVER dsygvd; the operator applies are this library's FP64 kernels.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -160,9 +160,14 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
     BY = h->rr2;
   }
   pt.lap("B Y");
-  RCHFSI_TRY(gram(h, Y, AY, h->Ha));
-  RCHFSI_TRY(gram(h, Y, BY, h->Hb));
-  pt.lap("Gram x2 (dgemm, lower)");
+  if (gram_i8_supported(h)) {   // rr3 holds the transposed digit planes until the rotation needs it
+    RCHFSI_TRY(gram_i8_full(h, Y, AY, h->B.present ? h->rr2 : nullptr, h->Ha, h->Hb, h->rr3, blk));
+    pt.lap("Gram x2 (INT8 tensor pipe, lower)");
+  } else {
+    RCHFSI_TRY(gram(h, Y, AY, h->Ha));
+    RCHFSI_TRY(gram(h, Y, BY, h->Hb));
+    pt.lap("Gram x2 (dgemm, lower)");
+  }
   // H_a E = H_b E Lambda, E^T H_b E = I, ascending (LAPACK dsygv type 1)
   CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
                                      CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,
@@ -180,9 +185,14 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
   const double *E = h->Ha;   // eigenvectors overwrite H_a, column-major
   double *T3 = h->rr3;
   // X = Y E
-  RCHFSI_TRY(rotate(h, Y, E, T3));
-  RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y, T3, blk, cudaMemcpyDeviceToDevice, st));
-  pt.lap("X = Y E (dgemm + copy)");
+  if (rotate_i8_supported(h)) {
+    RCHFSI_TRY(rotate_i8(h, Y, m, E, Y, T3, blk));            // in place; T3 holds the digit planes
+    pt.lap("X = Y E (INT8 tensor pipe)");
+  } else {
+    RCHFSI_TRY(rotate(h, Y, E, T3));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y, T3, blk, cudaMemcpyDeviceToDevice, st));
+    pt.lap("X = Y E (dgemm + copy)");
+  }
   const bool need_res = (G_out != nullptr) || (res_out != nullptr);
   if (need_res) {
     // AX and BX: either rotate the products already at hand, AX = (AY) E, BX = (BY) E (2 m N^2 flops each), or
@@ -202,6 +212,36 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
   }
   if (ritz_out && ritz_out != h->ritz_dev)
     RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(ritz_out, h->ritz_dev, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));
+  return RCHFSI_OK;
+}
+
+// Y <- Y E for a caller-given E (rchfsi_rotate): row panels through the panel buffer of the chunked variant.
+static void choose_row_panel(rchfsi_ctx *h) {
+  if (h->rr_rp == 0) {
+    int64_t rp = (int64_t)(3.0e9 / (8.0 * (double)h->N));
+    h->rr_rp = std::max<int64_t>(256, std::min<int64_t>(h->m, rp));
+  }
+}
+rchfsi_status rotate_in_place(rchfsi_ctx *h, double *Y, const double *E) {
+  const int64_t m = h->m;
+  const int32_t N = h->N;
+  if (!h->cublas) {
+    CUBLAS_CHECK(h, cublasCreate(&h->cublas));
+    CUBLAS_CHECK(h, cublasSetStream(h->cublas, h->stream));
+    CUBLAS_CHECK(h, cublasSetMathMode(h->cublas, CUBLAS_PEDANTIC_MATH));
+  }
+  choose_row_panel(h);
+  if (!h->rrp) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)h->rr_rp * N));
+  if (rotate_i8_supported(h)) return rotate_i8(h, Y, m, E, Y, h->rrp, sizeof(double) * (size_t)h->rr_rp * N);
+  const double one = 1.0, zero = 0.0;
+  for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
+    const int64_t rows = std::min<int64_t>(h->rr_rp, m - r0);
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_T, CUBLAS_OP_N, N, (int)rows, N, &one, E, N, Y + (size_t)r0 * N, N,
+                                &zero, h->rrp, N));
+    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y + (size_t)r0 * N, h->rrp, sizeof(double) * (size_t)rows * N,
+                                         cudaMemcpyDeviceToDevice, h->stream));
+    h->launches++;
+  }
   return RCHFSI_OK;
 }
 
@@ -232,10 +272,8 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) budget = std::max(budget, 0.33 * ((double)free_b - 12.0e9));   // 12 GB kept for the low-precision operator copies and scratch still to come
     int64_t cw = (int64_t)(budget / (16.0 * (double)m));
     cw = std::max<int64_t>(8, std::min<int64_t>(N, cw >= 48 ? cw / 48 * 48 : cw / 8 * 8));   // multiples of the FE column tile
-    int64_t rp = (int64_t)(3.0e9 / (8.0 * (double)N));
-    rp = std::max<int64_t>(256, std::min<int64_t>(m, rp));
     h->rr_cw = (int32_t)cw;
-    h->rr_rp = rp;
+    choose_row_panel(h);
   }
   // (each buffer has its own guard: the call may be repeated after the caller added workspace)
   if (!h->rrc1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)m * h->rr_cw));
@@ -249,23 +287,39 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     RCHFSI_TRY(column_sumsq(h, RCHFSI_FP64, Y, m, N, h->colnorm));
     RCHFSI_TRY(scale_columns_inv_norm(h, Y, m, N, h->colnorm));
   }
-  // Gram matrices, one column chunk of A Y / B Y at a time:  H[:, c0:c0+w] = Y^T (Op Y[:, c0:c0+w])
+  // Gram matrices, one column chunk of A Y / B Y at a time:  H[:, c0:c0+w] = Y^T (Op Y[:, c0:c0+w]).
+  // INT8 tensor pipe (rr_i8.cu) when the filter's blocks -- dead between two filters -- can hold the transposed digit
+  // planes of Y; cuBLAS dgemm otherwise (e.g. the Rayleigh-Ritz on the initial guess, before any filter ran).
+  bool g8 = false;
+  if (gram_i8_supported(h) && !h->run.active) {
+    std::vector<I8Buf> bufs;
+    if (h->RX) bufs.push_back({h->RX, h->RX_bytes});
+    if (h->RY) bufs.push_back({h->RY, h->RY_bytes});
+    if (h->Wa) bufs.push_back({h->Wa, h->Wa_bytes});
+    rchfsi_status gst = RCHFSI_OK;
+    g8 = gram_i8_begin(h, Y, bufs, cw, &gst);
+    if (gst != RCHFSI_OK) return gst;
+  }
   for (int32_t c0 = 0; c0 < N; c0 += cw) {
     const int32_t w = std::min(cw, N - c0);
     // lower triangle only (rows i >= c0 of this column slab): dsygvd reads nothing else
     RCHFSI_TRY(apply64(h, h->A.d, Y + c0, h->rrc1, w, N, w));
-    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc1, w, &zero,
-                                h->Ha + (size_t)c0 * N + c0, N));
+    if (g8) RCHFSI_TRY(gram_i8_slab(h, h->rrc1, w, w, c0, h->Ha));
+    else CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc1, w, &zero,
+                                     h->Ha + (size_t)c0 * N + c0, N));
     if (h->B.present) {
       RCHFSI_TRY(apply64(h, h->B.d, Y + c0, h->rrc2, w, N, w));
-      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc2, w, &zero,
-                                  h->Hb + (size_t)c0 * N + c0, N));
+      if (g8) RCHFSI_TRY(gram_i8_slab(h, h->rrc2, w, w, c0, h->Hb));
+      else CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc2, w, &zero,
+                                       h->Hb + (size_t)c0 * N + c0, N));
     } else {
-      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, Y + c0, N, &zero,
-                                  h->Hb + (size_t)c0 * N + c0, N));
+      if (g8) RCHFSI_TRY(gram_i8_slab(h, nullptr, 0, w, c0, h->Hb));
+      else CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, Y + c0, N, &zero,
+                                       h->Hb + (size_t)c0 * N + c0, N));
     }
     h->launches += 2;
   }
+  h->i8g.active = false;
   pt.lap("chunked: applies + Gram (lower)");
   CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
                                      CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,
@@ -282,13 +336,17 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   pt.lap("chunked: dsygvd");
   const double *E = h->Ha;
   // X = Y E in place, one row panel at a time (row-major rows r0.. are the columns r0.. of the N x m view)
-  for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
-    const int64_t rows = std::min<int64_t>(h->rr_rp, m - r0);
-    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_T, CUBLAS_OP_N, N, (int)rows, N, &one, E, N, Y + (size_t)r0 * N, N,
-                                &zero, h->rrp, N));
-    RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y + (size_t)r0 * N, h->rrp, sizeof(double) * (size_t)rows * N,
-                                         cudaMemcpyDeviceToDevice, st));
-    h->launches++;
+  if (rotate_i8_supported(h)) {
+    RCHFSI_TRY(rotate_i8(h, Y, m, E, Y, h->rrp, sizeof(double) * (size_t)h->rr_rp * N));   // the panel holds the digit planes
+  } else {
+    for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
+      const int64_t rows = std::min<int64_t>(h->rr_rp, m - r0);
+      CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_T, CUBLAS_OP_N, N, (int)rows, N, &one, E, N, Y + (size_t)r0 * N, N,
+                                  &zero, h->rrp, N));
+      RCHFSI_CUDA_CHECK(h, cudaMemcpyAsync(Y + (size_t)r0 * N, h->rrp, sizeof(double) * (size_t)rows * N,
+                                           cudaMemcpyDeviceToDevice, st));
+      h->launches++;
+    }
   }
   pt.lap("chunked: X = Y E (row panels)");
   if (G_out || res_out) {

@@ -1,0 +1,705 @@
+// Rayleigh-Ritz rotation X = Y E on the INT8 tensor pipe ("X = Y E", FP64 by
+// PAPER.md:25 footnote 1).  cuBLAS dgemm runs this product at the FP64 rate (34 TFLOP/s measured, 40 nominal); the INT8
+// tcgen05 path has >100x that rate, so an error-free split of the FP64 operands pays even at 28 integer products per
+// FP64 product (Ozaki-type scheme, restated here from the arithmetic, not from any code):
+//
+//   * every ROW i of Y and every COLUMN j of E gets a power-of-two scale 2^ea_i / 2^eb_j with |y| 2^-ea < 1, and its
+//     entries become 54-bit fixed-point integers q = rint(y 2^(54 - ea));  the largest entry of the row keeps all 53
+//     mantissa bits, smaller entries are rounded at 2^-54 of the row maximum (absolute, like a fixed-point dot product);
+//   * q is written in S = 7 balanced base-256 digits d_0 (most significant) .. d_6, each an int8 in [-128, 127]:
+//     q = sum_s d_s 256^(6-s), exactly;
+//   * digit planes multiply exactly on the tensor pipe (tcgen05.mma kind::i8, INT32 accumulators): all pairs (s, t) of
+//     one anti-diagonal d = s + t share the weight 2^(-12-8d) and ONE accumulator; the pairs with d <= 6 are kept
+//     (28 products), the dropped ones weigh <= 2^-54 each relative to (row max)(column max);
+//     INT32 is exact while (d+1) K 2^14 < 2^31, i.e. K = N <= 18000;
+//   * epilogue: X_ij = 2^(ea_i + eb_j - 12) sum_d acc_d 2^(-8d) in FP64 (Horner from d = 6).
+//
+// Kernels: i8_slice_kernel (digit planes of a row chunk of Y, or of the columns of E), i8_rotate_kernel (TMA ->
+// shared-memory rings -> tcgen05.mma kind::i8 -> 7 TMEM accumulators -> FP64 recombination).  The rotation runs in
+// place, one row chunk at a time: once the digit planes of a chunk exist its rows of Y are dead.
+#include <algorithm>
+#include <vector>
+#include "common.cuh"
+#include "tc_common.cuh"
+
+namespace rchfsi {
+namespace {
+
+using namespace tc;
+
+constexpr int I8_S = 7;                 // digit planes per operand
+constexpr int I8_BN = 64;               // output columns per CTA (7 accumulators x 64 = 448 of 512 TMEM columns)
+constexpr int I8_A_TILE = 128 * 128;    // 128 rows x 128 B of K
+constexpr int I8_B_TILE = I8_BN * 128;
+constexpr int I8_NA = 6;                // A ring slots (tiles are consumed and released in order)
+constexpr int I8_SMEM = I8_NA * I8_A_TILE + 2 * I8_S * I8_B_TILE + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int32_t I8_NAN_ROW = 0x7fffffff;
+
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// instruction descriptor: S32 accumulate (2 at bit 4), signed 8-bit A and B (1 at bits 7 and 10), both K-major
+__host__ __device__ constexpr uint32_t make_idesc_i8(int M, int N) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// One warp per row of V ([rows][K], row pitch ld): row exponent, then the 7 digit planes planes[s][row][Kp].
+// Columns K..Kp-1 of the planes are zero (Kp = K rounded up to 16: TMA row pitch).
+__global__ void __launch_bounds__(256) i8_slice_kernel(const double *__restrict__ V, int64_t ld, int64_t rows, int32_t K,
+                                                       int32_t Kp, int8_t *__restrict__ planes, int64_t plane_rows,
+                                                       int32_t *__restrict__ expo) {
+  const int lane = threadIdx.x & 31;
+  const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (row >= rows) return;
+  const double *v = V + row * ld;
+  double mx = 0.0;
+  bool bad = false;
+  for (int k = lane; k < K; k += 32) {
+    const double a = fabs(v[k]);
+    bad |= !(a <= 1.7976931348623157e308);      // inf or NaN
+    mx = fmax(mx, a);
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    bad |= __shfl_xor_sync(0xffffffffu, (int)bad, o) != 0;
+  }
+  const int e = mx > 0.0 ? ilogb(mx) + 1 : 0;   // |v| 2^-e < 1
+  if (lane == 0) expo[row] = bad ? I8_NAN_ROW : e;
+  const size_t plane = (size_t)plane_rows * Kp;
+  int8_t *out = planes + (size_t)row * Kp;
+  for (int k4 = lane * 4; k4 < Kp; k4 += 128) {
+    uint32_t packed[I8_S];
+#pragma unroll
+    for (int s = 0; s < I8_S; ++s) packed[s] = 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int k = k4 + u;
+      long long q = (k < K && !bad) ? __double2ll_rn(scalbn(v[k], 54 - e)) : 0ll;
+#pragma unroll
+      for (int s = I8_S - 1; s >= 0; --s) {     // least significant digit first
+        const int d = (int)(int8_t)(q & 0xff);
+        q = (q - d) >> 8;
+        packed[s] |= (uint32_t)(d & 0xff) << (8 * u);
+      }
+    }
+#pragma unroll
+    for (int s = 0; s < I8_S; ++s) *reinterpret_cast<uint32_t *>(out + s * plane + k4) = packed[s];
+  }
+}
+
+struct I8Params {
+  double *Out;            // [rows][ldo] FP64, first row = first row of the chunk
+  int64_t ldo;
+  const int32_t *ea;      // [rows] row exponents of the chunk
+  const int32_t *eb;      // [N] column exponents of E
+  int32_t rows;           // rows in this chunk (= plane rows of the A planes)
+  int32_t N;              // columns of E / of the output
+  int32_t num_k_blocks;   // ceil(K / 128)
+};
+
+// grid (column tiles, row blocks); 192 threads: warp 0 TMA, warp 1 MMA, warps 2-5 epilogue (TMEM lane quarter warp % 4)
+__global__ void __launch_bounds__(192, 1) i8_rotate_kernel(const __grid_constant__ CUtensorMap tmA,
+                                                           const __grid_constant__ CUtensorMap tmB, I8Params p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t *As = smem;
+  uint8_t *Bs = smem + I8_NA * I8_A_TILE;
+  uint64_t *a_full = reinterpret_cast<uint64_t *>(Bs + 2 * I8_S * I8_B_TILE);
+  uint64_t *a_empty = a_full + I8_NA;
+  uint64_t *b_full = a_empty + I8_NA;
+  uint64_t *b_empty = b_full + 2;
+  uint64_t *accum_bar = b_empty + 2;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(accum_bar + 1);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int j0 = blockIdx.x * I8_BN;
+  const int i0 = blockIdx.y * 128;
+  const int nkb = p.num_k_blocks;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB);
+    for (int s = 0; s < I8_NA; ++s) {
+      mbar_init(a_full + s, 1);
+      mbar_init(a_empty + s, 1);
+    }
+    for (int g = 0; g < 2; ++g) {
+      mbar_init(b_full + g, 1);
+      mbar_init(b_empty + g, 1);
+    }
+    mbar_init(accum_bar, 1);
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===== TMA producer: per K block the 7 digit planes of the E tile (one group barrier), then the 7 of the Y tile
+    for (int kb = 0; kb < nkb; ++kb) {
+      const int g = kb & 1;
+      const int k0 = kb * 128;
+      mbar_wait(b_empty + g, ((kb >> 1) & 1) ^ 1);
+      if (elect_one()) {
+        mbar_expect_tx(b_full + g, I8_S * I8_B_TILE);
+#pragma unroll
+        for (int t = 0; t < I8_S; ++t) tma_load_2d(Bs + (g * I8_S + t) * I8_B_TILE, &tmB, b_full + g, k0, t * p.N + j0);
+      }
+      __syncwarp();
+      for (int s = 0; s < I8_S; ++s) {
+        const int ia = kb * I8_S + s;
+        const int slot = ia % I8_NA;
+        mbar_wait(a_empty + slot, ((ia / I8_NA) & 1) ^ 1);
+        if (elect_one()) {
+          mbar_expect_tx(a_full + slot, I8_A_TILE);
+          tma_load_2d(As + slot * I8_A_TILE, &tmA, a_full + slot, k0, s * p.rows + i0);
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: for s, for t <= 6 - s: acc[s + t] += A_s B_t^T (4 K steps of 32 inside the 128-byte rows)
+    constexpr uint32_t idesc = make_idesc_i8(128, I8_BN);
+    const uint64_t da0 = make_smem_desc(smem_u32(As), 16, 1024, 2);
+    const uint64_t db0 = make_smem_desc(smem_u32(Bs), 16, 1024, 2);
+    for (int kb = 0; kb < nkb; ++kb) {
+      const int g = kb & 1;
+      mbar_wait(b_full + g, (kb >> 1) & 1);
+      for (int s = 0; s < I8_S; ++s) {
+        const int ia = kb * I8_S + s;
+        const int slot = ia % I8_NA;
+        mbar_wait(a_full + slot, (ia / I8_NA) & 1);
+        tc_fence_after();
+        if (elect_one()) {
+          const uint64_t da = da0 + (uint32_t)((slot * I8_A_TILE) >> 4);
+          for (int t = 0; t < I8_S - s; ++t) {
+            const uint64_t db = db0 + (uint32_t)(((g * I8_S + t) * I8_B_TILE) >> 4);
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+              umma_i8(tmem_base + (uint32_t)((s + t) * I8_BN), da + 2 * q, db + 2 * q, idesc,
+                      (kb > 0 || s > 0 || q > 0) ? 1u : 0u);
+          }
+          umma_commit(a_empty + slot);
+          if (s == I8_S - 1) umma_commit(b_empty + g);
+        }
+        __syncwarp();
+      }
+    }
+    if (elect_one()) umma_commit(accum_bar);
+    __syncwarp();
+  } else {
+    // ===== epilogue: thread = output row (TMEM lane), 8 columns at a time
+    const int qd = warp & 3;
+    const int r = 32 * qd + lane;
+    const int64_t row = (int64_t)i0 + r;
+    const bool rok = row < p.rows;
+    const int ea = rok ? p.ea[row] : 0;
+    double *orow = p.Out + row * p.ldo;
+    mbar_wait(accum_bar, 0);
+    tc_fence_after();
+#pragma unroll 1
+    for (int c0 = 0; c0 < I8_BN; c0 += 8) {
+      uint32_t a[I8_S][8];
+#pragma unroll
+      for (int d = 0; d < I8_S; ++d) tmem_ld_32x8(tmem_base + ((uint32_t)(32 * qd) << 16) + (uint32_t)(d * I8_BN + c0), a[d]);
+      tmem_ld_wait();
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int j = j0 + c0 + u;
+        if (rok && j < p.N) {
+          double v = (double)(int32_t)a[I8_S - 1][u];
+#pragma unroll
+          for (int d = I8_S - 2; d >= 0; --d) v = fma(v, 0.00390625, (double)(int32_t)a[d][u]);
+          const int eb = p.eb[j];
+          const bool nan = ea == I8_NAN_ROW || eb == I8_NAN_ROW;
+          orow[j] = nan ? __longlong_as_double(0x7ff8000000000000ll) : scalbn(v, ea + eb - 12);
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tmem_base, 512);
+}
+
+// ------------------------------------------------------------------------------------------------ Gram products
+// H = Y^T Z (contraction over the m rows) with the same digit split, per-COLUMN scales (a column of Y / Z is a row of
+// the K-major operand Y^T / Z^T), transposed digit planes planes[s][column][row], and INT32 accumulators flushed into
+// FP64 registers every I8_FLUSH K blocks (7 * 16384 * 2^14 < 2^31).
+constexpr int I8_FLUSH = 128;           // K blocks of 128 rows between two flushes
+
+struct I8Maps { CUtensorMap m[I8_S]; };
+struct I8Planes { int8_t *p[I8_S]; };
+
+// mx[j] = max_i |V[i][j]| as a bit pattern (non-negative doubles order like integers; NaN / inf give >= 0x7ff0...)
+__global__ void __launch_bounds__(256) i8_colmax_kernel(const double *__restrict__ V, int64_t ld, int64_t rows, int32_t cols,
+                                                        int64_t rows_per_cta, unsigned long long *mx) {
+  const int64_t r0 = blockIdx.x * rows_per_cta;
+  const int64_t r1 = min(rows, r0 + rows_per_cta);
+  for (int j = threadIdx.x; j < cols; j += blockDim.x) {
+    unsigned long long best = 0ull;
+    for (int64_t i = r0; i < r1; ++i) best = max(best, (unsigned long long)__double_as_longlong(fabs(V[i * ld + j])));
+    atomicMax(mx + j, best);
+  }
+}
+
+// Transposed digit planes of the rows [r0, r0 + rows) of V ([.][cols], pitch ld): planes.p[s][col * Rp + (row - r0)].
+// Block = 128 rows x 32 columns through a padded shared tile; rows beyond the chunk are written as zeros up to Rp.
+__global__ void __launch_bounds__(256) i8_slice_t_kernel(const double *__restrict__ V, int64_t ld, int64_t r0, int64_t rows,
+                                                         int32_t cols, int64_t Rp, const unsigned long long *__restrict__ mx,
+                                                         I8Planes planes, int32_t *__restrict__ expo) {
+  __shared__ uint32_t tile[I8_S][32][33];
+  const int lane = threadIdx.x & 31;
+  const int w = threadIdx.x >> 5;
+  const int col = blockIdx.x * 32 + lane;
+  const bool cok = col < cols;
+  const unsigned long long bits = cok ? mx[col] : 0ull;
+  const bool bad = bits >= 0x7ff0000000000000ull;
+  const double cm = __longlong_as_double((long long)bits);
+  const int e = (cm > 0.0 && !bad) ? ilogb(cm) + 1 : 0;
+  if (blockIdx.y == 0 && w == 0 && cok && expo) expo[col] = bad ? I8_NAN_ROW : e;
+#pragma unroll 4
+  for (int i = 0; i < 16; ++i) {
+    const int rl = w + 8 * i;
+    const int64_t r = (int64_t)blockIdx.y * 128 + rl;
+    long long q = (cok && !bad && r < rows) ? __double2ll_rn(scalbn(V[(r0 + r) * ld + col], 54 - e)) : 0ll;
+#pragma unroll
+    for (int s = I8_S - 1; s >= 0; --s) {
+      const int d = (int)(int8_t)(q & 0xff);
+      q = (q - d) >> 8;
+      reinterpret_cast<uint8_t *>(&tile[s][lane][0])[rl] = (uint8_t)d;
+    }
+  }
+  __syncthreads();
+  const int64_t roff = (int64_t)blockIdx.y * 128 + lane * 4;
+  for (int idx = w; idx < I8_S * 32; idx += 8) {
+    const int s = idx >> 5, c = idx & 31;
+    const int cg = blockIdx.x * 32 + c;
+    if (cg < cols && roff < Rp) *reinterpret_cast<uint32_t *>(planes.p[s] + (size_t)cg * Rp + roff) = tile[s][c][lane];
+  }
+}
+
+struct I8GramParams {
+  double *Hpart;          // [KS][Nz][N] FP64 partial sums (unscaled), element (ks, b, a)
+  int32_t N;              // columns of Y (M side, a)
+  int32_t Nz;             // columns of Z in this slab (N side, b)
+  int32_t zc0;            // global column of Z's first column: only tiles with rows a >= zc0 + b are formed
+  int32_t num_k_blocks;   // ceil(rows / 128) of this row chunk
+  int32_t accumulate;     // add to Hpart (row chunks after the first)
+};
+
+// grid (b tiles of 64, a tiles of 128, K splits); same warp roles as i8_rotate_kernel
+__global__ void __launch_bounds__(192, 1) i8_gram_kernel(const __grid_constant__ I8Maps mapsA, const __grid_constant__ I8Maps mapsB,
+                                                         I8GramParams p) {
+  const int b0 = blockIdx.x * I8_BN;
+  const int a0 = blockIdx.y * 128;
+  if (a0 + 127 < p.zc0 + b0) return;          // tile entirely above the diagonal: never read
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t *As = smem;
+  uint8_t *Bs = smem + I8_NA * I8_A_TILE;
+  uint64_t *a_full = reinterpret_cast<uint64_t *>(Bs + 2 * I8_S * I8_B_TILE);
+  uint64_t *a_empty = a_full + I8_NA;
+  uint64_t *b_full = a_empty + I8_NA;
+  uint64_t *b_empty = b_full + 2;
+  uint64_t *accum_bar = b_empty + 2;
+  uint64_t *drained_bar = accum_bar + 1;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(drained_bar + 1);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int ks = gridDim.z;
+  const int kb0 = (int)((int64_t)p.num_k_blocks * blockIdx.z / ks);
+  const int nk = (int)((int64_t)p.num_k_blocks * (blockIdx.z + 1) / ks) - kb0;
+
+  if (warp == 0 && lane == 0) {
+    for (int s = 0; s < I8_S; ++s) {
+      tma_prefetch_desc(&mapsA.m[s]);
+      tma_prefetch_desc(&mapsB.m[s]);
+    }
+    for (int s = 0; s < I8_NA; ++s) {
+      mbar_init(a_full + s, 1);
+      mbar_init(a_empty + s, 1);
+    }
+    for (int g = 0; g < 2; ++g) {
+      mbar_init(b_full + g, 1);
+      mbar_init(b_empty + g, 1);
+    }
+    mbar_init(accum_bar, 1);
+    mbar_init(drained_bar, 4);
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    for (int c = 0; c < nk; ++c) {
+      const int g = c & 1;
+      const int k0 = (kb0 + c) * 128;
+      mbar_wait(b_empty + g, ((c >> 1) & 1) ^ 1);
+      if (elect_one()) {
+        mbar_expect_tx(b_full + g, I8_S * I8_B_TILE);
+#pragma unroll
+        for (int t = 0; t < I8_S; ++t) tma_load_2d(Bs + (g * I8_S + t) * I8_B_TILE, &mapsB.m[t], b_full + g, k0, b0);
+      }
+      __syncwarp();
+      for (int s = 0; s < I8_S; ++s) {
+        const int ia = c * I8_S + s;
+        const int slot = ia % I8_NA;
+        mbar_wait(a_empty + slot, ((ia / I8_NA) & 1) ^ 1);
+        if (elect_one()) {
+          mbar_expect_tx(a_full + slot, I8_A_TILE);
+          tma_load_2d(As + slot * I8_A_TILE, &mapsA.m[s], a_full + slot, k0, a0);
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp == 1) {
+    constexpr uint32_t idesc = make_idesc_i8(128, I8_BN);
+    const uint64_t da0 = make_smem_desc(smem_u32(As), 16, 1024, 2);
+    const uint64_t db0 = make_smem_desc(smem_u32(Bs), 16, 1024, 2);
+    for (int c = 0; c < nk; ++c) {
+      const int g = c & 1;
+      const int cr = c % I8_FLUSH;             // position inside the flush round
+      if (c > 0 && cr == 0) {                  // the epilogue has read the accumulators of the previous round
+        mbar_wait(drained_bar, ((c / I8_FLUSH) - 1) & 1);
+        tc_fence_after();
+      }
+      mbar_wait(b_full + g, (c >> 1) & 1);
+      for (int s = 0; s < I8_S; ++s) {
+        const int ia = c * I8_S + s;
+        const int slot = ia % I8_NA;
+        mbar_wait(a_full + slot, (ia / I8_NA) & 1);
+        tc_fence_after();
+        if (elect_one()) {
+          const uint64_t da = da0 + (uint32_t)((slot * I8_A_TILE) >> 4);
+          for (int t = 0; t < I8_S - s; ++t) {
+            const uint64_t db = db0 + (uint32_t)(((g * I8_S + t) * I8_B_TILE) >> 4);
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+              umma_i8(tmem_base + (uint32_t)((s + t) * I8_BN), da + 2 * q, db + 2 * q, idesc,
+                      (cr > 0 || s > 0 || q > 0) ? 1u : 0u);
+          }
+          umma_commit(a_empty + slot);
+          if (s == I8_S - 1) {
+            umma_commit(b_empty + g);
+            if (cr == I8_FLUSH - 1 || c == nk - 1) umma_commit(accum_bar);
+          }
+        }
+        __syncwarp();
+      }
+    }
+  } else {
+    const int qd = warp & 3;
+    const int r = 32 * qd + lane;
+    double acc[I8_BN];
+#pragma unroll
+    for (int u = 0; u < I8_BN; ++u) acc[u] = 0.0;
+    const int rounds = (nk + I8_FLUSH - 1) / I8_FLUSH;
+    for (int rd = 0; rd < rounds; ++rd) {
+      mbar_wait(accum_bar, rd & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c0 = 0; c0 < I8_BN; c0 += 8) {
+        uint32_t a[I8_S][8];
+#pragma unroll
+        for (int d = 0; d < I8_S; ++d) tmem_ld_32x8(tmem_base + ((uint32_t)(32 * qd) << 16) + (uint32_t)(d * I8_BN + c0), a[d]);
+        tmem_ld_wait();
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          double v = (double)(int32_t)a[I8_S - 1][u];
+#pragma unroll
+          for (int d = I8_S - 2; d >= 0; --d) v = fma(v, 0.00390625, (double)(int32_t)a[d][u]);
+          acc[c0 + u] += v;
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(drained_bar);
+    }
+    const int a = a0 + r;
+    if (a < p.N) {
+#pragma unroll
+      for (int u = 0; u < I8_BN; ++u) {
+        const int b = b0 + u;
+        if (b < p.Nz) {
+          double *dst = p.Hpart + ((size_t)blockIdx.z * p.Nz + b) * p.N + a;
+          *dst = p.accumulate ? *dst + acc[u] : acc[u];
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tmem_base, 512);
+}
+
+// H(a, zc0 + b) = 2^(ea_a + eb_b - 12) sum_ks Hpart[ks][b][a] for the lower triangle a >= zc0 + b (column-major H)
+__global__ void __launch_bounds__(256) i8_gram_finish_kernel(const double *__restrict__ Hpart, int32_t KS, int32_t N, int32_t Nz,
+                                                             int32_t zc0, const int32_t *__restrict__ ea,
+                                                             const int32_t *__restrict__ eb, double *__restrict__ H) {
+  const int b = blockIdx.y;
+  const int eb_ = eb[b];
+  for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < N; a += gridDim.x * blockDim.x) {
+    if (a < zc0 + b) continue;
+    double v = 0.0;
+    for (int k = 0; k < KS; ++k) v += Hpart[((size_t)k * Nz + b) * N + a];
+    const int ea_ = ea[a];
+    const bool nan = ea_ == I8_NAN_ROW || eb_ == I8_NAN_ROW;
+    H[(size_t)(zc0 + b) * N + a] = nan ? __longlong_as_double(0x7ff8000000000000ll) : scalbn(v, ea_ + eb_ - 12);
+  }
+}
+
+}  // namespace
+
+bool rotate_i8_supported(const rchfsi_ctx *h) {
+  if (h->knobs.rr_split == 0) return false;
+  if (h->N > 16384) return false;                         // INT32 exactness: 7 N 2^14 < 2^31
+  if (h->knobs.rr_split > 0) return h->N >= 16;              // forced (tests at small sizes)
+  return h->N >= 256 && h->m >= 8192;                     // where it beats dgemm
+}
+
+size_t rotate_i8_fixed_bytes(int32_t N) {
+  const size_t Kp = ((size_t)N + 15) / 16 * 16;
+  return (size_t)I8_S * N * Kp + 4 * (size_t)N + 1024;
+}
+
+// Out[r][:] = In[r][:] E for r < rows (E column-major N x N); Out may be In.  `scratch` holds the digit planes and
+// exponents of one row chunk: the more rows fit, the fewer chunk launches.
+rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const double *E, double *Out, void *scratch,
+                        size_t scratch_bytes) {
+  const int32_t N = h->N;
+  const int32_t Kp = (N + 15) / 16 * 16;
+  if (!h->i8_E) RCHFSI_TRY(dev_alloc(h, &h->i8_E, rotate_i8_fixed_bytes(h->N_cap)));
+  int8_t *Eplanes = reinterpret_cast<int8_t *>(h->i8_E);
+  int32_t *eb = reinterpret_cast<int32_t *>(Eplanes + ((size_t)I8_S * N * Kp + 255) / 256 * 256);
+  const size_t per_row = (size_t)I8_S * Kp + 4;
+  int64_t R = (int64_t)((scratch_bytes > 4096 ? scratch_bytes - 4096 : 0) / per_row);
+  R = std::min<int64_t>(R, rows);
+  if (h->knobs.rr_i8_rows > 0) R = std::min<int64_t>(R, h->knobs.rr_i8_rows);
+  if (R >= 128) R = R / 128 * 128;
+  if (R < 1 || R > 0x7fffff00 / I8_S) R = std::min<int64_t>(R, 0x7fffff00 / I8_S);
+  if (R < 1) { h->err = "rotate_i8: scratch too small"; return RCHFSI_EINVAL; }
+  int8_t *Aplanes = reinterpret_cast<int8_t *>(scratch);
+  int32_t *ea = reinterpret_cast<int32_t *>(Aplanes + ((size_t)I8_S * R * Kp + 255) / 256 * 256);
+  RCHFSI_TRY(ensure_func_smem(h, (const void *)i8_rotate_kernel, I8_SMEM));
+  cudaStream_t st = h->stream;
+  // digit planes of the columns of E (column-major: column j is contiguous, i.e. a "row" of the slicing kernel)
+  i8_slice_kernel<<<(unsigned)cdiv(N, 8), 256, 0, st>>>(E, N, N, N, Kp, Eplanes, N, eb);
+  LAUNCH_CHECK(h);
+  CUtensorMap tmB;
+  if (!get_tmap_2d(h, &tmB, Eplanes, 1, false, (uint64_t)I8_S * N, (uint64_t)Kp, (uint64_t)Kp, 128, I8_BN)) {
+    h->err = "rotate_i8: cuTensorMapEncodeTiled failed (E planes)";
+    return RCHFSI_ECUDA;
+  }
+  for (int64_t r0 = 0; r0 < rows; r0 += R) {
+    const int64_t rc = std::min<int64_t>(R, rows - r0);
+    i8_slice_kernel<<<(unsigned)cdiv(rc, 8), 256, 0, st>>>(In + (size_t)r0 * N, N, rc, N, Kp, Aplanes, rc, ea);
+    LAUNCH_CHECK(h);
+    CUtensorMap tmA;
+    if (!get_tmap_2d(h, &tmA, Aplanes, 1, false, (uint64_t)I8_S * rc, (uint64_t)Kp, (uint64_t)Kp, 128, 128)) {
+      h->err = "rotate_i8: cuTensorMapEncodeTiled failed (Y planes)";
+      return RCHFSI_ECUDA;
+    }
+    I8Params p{Out + (size_t)r0 * N, N, ea, eb, (int32_t)rc, N, (int32_t)cdiv(N, 128)};
+    dim3 grid((unsigned)cdiv(N, I8_BN), (unsigned)cdiv(rc, 128));
+    i8_rotate_kernel<<<grid, 192, I8_SMEM, st>>>(tmA, tmB, p);
+    LAUNCH_CHECK(h);
+  }
+  return RCHFSI_OK;
+}
+
+// ---------------------------------------------------------------------------------------- Gram products (host side)
+bool gram_i8_supported(const rchfsi_ctx *h) {
+  if (h->knobs.rr_gram_i8 == 0) return false;
+  if (h->knobs.rr_gram_i8 > 0) return h->N >= 16;        // forced (tests at small sizes)
+  return h->N >= 256 && h->m >= 8192;
+}
+
+namespace {
+
+bool carve(std::vector<I8Buf> &bufs, size_t bytes, void **out) {
+  for (I8Buf &b : bufs) {
+    const size_t off = (256 - (reinterpret_cast<uintptr_t>(b.ptr) & 255)) & 255;
+    if (b.bytes >= bytes + off) {
+      *out = reinterpret_cast<uint8_t *>(b.ptr) + off;
+      b.ptr = reinterpret_cast<uint8_t *>(*out) + bytes;
+      b.bytes -= bytes + off;
+      return true;
+    }
+  }
+  return false;
+}
+
+rchfsi_status i8_fixed(rchfsi_ctx *h) {   // column maxima and exponents of Y and Z
+  if (!h->i8_cols) RCHFSI_TRY(dev_alloc(h, &h->i8_cols, (size_t)h->N_cap * 24 + 1024));
+  return RCHFSI_OK;
+}
+unsigned long long *mx_of(rchfsi_ctx *h, int which) { return reinterpret_cast<unsigned long long *>(h->i8_cols) + (size_t)which * h->N_cap; }
+int32_t *exp_of(rchfsi_ctx *h, int which) { return reinterpret_cast<int32_t *>(mx_of(h, 2)) + (size_t)which * h->N_cap; }
+
+rchfsi_status colmax(rchfsi_ctx *h, const double *V, int64_t ld, int32_t cols, unsigned long long *mx) {
+  RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(mx, 0, sizeof(unsigned long long) * cols, h->stream));
+  int64_t ctas = std::min<int64_t>(h->m, 148 * 8);
+  const int64_t rows = cdiv(h->m, ctas);
+  ctas = cdiv(h->m, rows);
+  i8_colmax_kernel<<<(unsigned)ctas, 256, 0, h->stream>>>(V, ld, h->m, cols, rows, mx);
+  LAUNCH_CHECK(h);
+  return RCHFSI_OK;
+}
+
+rchfsi_status slice_t(rchfsi_ctx *h, const double *V, int64_t ld, int64_t r0, int64_t rows, int32_t cols, int64_t Rp,
+                      const unsigned long long *mx, const I8Planes &pl, int32_t *expo) {
+  dim3 grid((unsigned)cdiv(cols, 32), (unsigned)cdiv(rows, 128));
+  i8_slice_t_kernel<<<grid, 256, 0, h->stream>>>(V, ld, r0, rows, cols, Rp, mx, pl, expo);
+  LAUNCH_CHECK(h);
+  return RCHFSI_OK;
+}
+
+bool plane_maps(rchfsi_ctx *h, I8Maps *maps, const I8Planes &pl, int32_t cols, int64_t Rp, uint32_t box_rows) {
+  for (int s = 0; s < I8_S; ++s)
+    if (!get_tmap_2d(h, &maps->m[s], pl.p[s], 1, false, (uint64_t)cols, (uint64_t)Rp, (uint64_t)Rp, 128, box_rows)) return false;
+  return true;
+}
+
+// one slab: Hpart (+)= Y^T Z over the K blocks of this row chunk, then (last chunk) H = scaled sum
+rchfsi_status gram_launch(rchfsi_ctx *h, const I8Planes &yp, const I8Planes &zp, int64_t Rp, int64_t rows, int32_t Nz, int32_t zc0,
+                          bool accumulate, int32_t KS) {
+  I8Maps ma, mb;
+  if (!plane_maps(h, &ma, yp, h->N, Rp, 128) || !plane_maps(h, &mb, zp, Nz, Rp, I8_BN)) {
+    h->err = "gram_i8: cuTensorMapEncodeTiled failed";
+    return RCHFSI_ECUDA;
+  }
+  RCHFSI_TRY(ensure_func_smem(h, (const void *)i8_gram_kernel, I8_SMEM));
+  I8GramParams p{reinterpret_cast<double *>(h->i8_hpart), h->N, Nz, zc0, (int32_t)cdiv(rows, 128), accumulate ? 1 : 0};
+  dim3 grid((unsigned)cdiv(Nz, I8_BN), (unsigned)cdiv(h->N, 128), (unsigned)KS);
+  i8_gram_kernel<<<grid, 192, I8_SMEM, h->stream>>>(ma, mb, p);
+  LAUNCH_CHECK(h);
+  return RCHFSI_OK;
+}
+
+int32_t choose_ks(int32_t N, int32_t Nz, int32_t zc0, int64_t rows) {
+  int64_t tiles = 0;
+  for (int a0 = 0; a0 < N; a0 += 128)
+    for (int b0 = 0; b0 < Nz; b0 += I8_BN) tiles += (a0 + 127 >= zc0 + b0);
+  const int64_t nkb = cdiv(rows, 128);
+  int64_t ks = cdiv((int64_t)4 * 148, std::max<int64_t>(tiles, 1));
+  return (int32_t)std::max<int64_t>(1, std::min<int64_t>({ks, (int64_t)32, nkb}));
+}
+
+rchfsi_status ensure_hpart(rchfsi_ctx *h, size_t bytes) {
+  if (h->i8_hpart_bytes < bytes) {
+    RCHFSI_TRY(dev_alloc(h, &h->i8_hpart, bytes));
+    h->i8_hpart_bytes = bytes;
+  }
+  return RCHFSI_OK;
+}
+
+rchfsi_status gram_finish(rchfsi_ctx *h, int32_t KS, int32_t Nz, int32_t zc0, const int32_t *ea, const int32_t *eb, double *H) {
+  dim3 grid((unsigned)cdiv(h->N, 256), (unsigned)Nz);
+  i8_gram_finish_kernel<<<grid, 256, 0, h->stream>>>(reinterpret_cast<const double *>(h->i8_hpart), KS, h->N, Nz, zc0, ea, eb, H);
+  LAUNCH_CHECK(h);
+  return RCHFSI_OK;
+}
+
+}  // namespace
+
+// workspace the INT8 Rayleigh-Ritz products hold beyond the blocks they borrow (planner: automatic choice only)
+size_t rr_i8_plan_bytes(int64_t m, int32_t N) {
+  if (N < 256 || m < 8192 || N > 16384) return 0;
+  auto al = [](size_t b) { return (b + 255) / 256 * 256; };
+  return al(rotate_i8_fixed_bytes(N)) + al((size_t)N * 24 + 1024) + al(sizeof(double) * (size_t)choose_ks(N, N, 0, m) * N * N);
+}
+
+// Full-block variant: H_a = Y^T (AY), H_b = Y^T (BY) (BY == NULL: Y^T Y), lower triangles, column-major.  `scratch`
+// holds the transposed digit planes of one row chunk of Y and of Z.
+rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, const double *BY, double *Ha, double *Hb,
+                           void *scratch, size_t scratch_bytes) {
+  const int32_t N = h->N;
+  const int64_t m = h->m;
+  RCHFSI_TRY(i8_fixed(h));
+  // rows per chunk: 2 x 7 planes of N x Rp bytes
+  int64_t R = (int64_t)((scratch_bytes > 8192 ? scratch_bytes - 8192 : 0) / ((size_t)2 * I8_S * N));
+  R = std::min<int64_t>(R / 128 * 128, (m + 127) / 128 * 128);
+  if (h->knobs.rr_i8_rows > 0) R = std::min<int64_t>(R, (h->knobs.rr_i8_rows + 127) / 128 * 128);
+  if (R < 128) { h->err = "gram_i8: scratch too small"; return RCHFSI_EINVAL; }
+  const int64_t Rp = R;
+  I8Planes yp, zp;
+  uint8_t *base = reinterpret_cast<uint8_t *>(scratch);
+  base += (256 - (reinterpret_cast<uintptr_t>(base) & 255)) & 255;
+  for (int s = 0; s < I8_S; ++s) {
+    yp.p[s] = reinterpret_cast<int8_t *>(base + (size_t)s * N * Rp);
+    zp.p[s] = reinterpret_cast<int8_t *>(base + (size_t)(I8_S + s) * N * Rp);
+  }
+  const int32_t KS = choose_ks(N, N, 0, R);
+  RCHFSI_TRY(ensure_hpart(h, sizeof(double) * (size_t)KS * N * N));
+  RCHFSI_TRY(colmax(h, Y, N, N, mx_of(h, 0)));
+  for (int prod = 0; prod < 2; ++prod) {
+    const double *Z = prod == 0 ? AY : BY;
+    const bool same = Z == nullptr;                       // Y^T Y
+    if (!same) RCHFSI_TRY(colmax(h, Z, N, N, mx_of(h, 1)));
+    for (int64_t r0 = 0; r0 < m; r0 += R) {
+      const int64_t rc = std::min<int64_t>(R, m - r0);
+      RCHFSI_TRY(slice_t(h, Y, N, r0, rc, N, Rp, mx_of(h, 0), yp, exp_of(h, 0)));
+      if (!same) RCHFSI_TRY(slice_t(h, Z, N, r0, rc, N, Rp, mx_of(h, 1), zp, exp_of(h, 1)));
+      RCHFSI_TRY(gram_launch(h, yp, same ? yp : zp, Rp, rc, N, 0, r0 > 0, KS));
+    }
+    RCHFSI_TRY(gram_finish(h, KS, N, 0, exp_of(h, 0), same ? exp_of(h, 0) : exp_of(h, 1), prod == 0 ? Ha : Hb));
+  }
+  return RCHFSI_OK;
+}
+
+// Column-slab variant (memory-light Rayleigh-Ritz): the transposed planes of ALL rows of Y are built once into the
+// caller's buffers (the filter's dead blocks), then every column slab Z_c = Op Y[:, c0:c0+w] contributes
+// H[:, c0:c0+w] = Y^T Z_c.  Returns false (nothing launched) when the buffers cannot hold the planes.
+bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int32_t max_w, rchfsi_status *st) {
+  *st = RCHFSI_OK;
+  const int32_t N = h->N;
+  const int64_t m = h->m;
+  const int64_t Rp = (m + 127) / 128 * 128;
+  I8GramState &g = h->i8g;
+  g.active = false;
+  for (int s = 0; s < I8_S; ++s)
+    if (!carve(bufs, (size_t)N * Rp, reinterpret_cast<void **>(&g.yp[s]))) return false;
+  for (int s = 0; s < I8_S; ++s)
+    if (!carve(bufs, (size_t)max_w * Rp, reinterpret_cast<void **>(&g.zp[s]))) return false;
+  g.Rp = Rp;
+  g.max_w = max_w;
+  if ((*st = i8_fixed(h)) != RCHFSI_OK) return false;
+  if ((*st = colmax(h, Y, N, N, mx_of(h, 0))) != RCHFSI_OK) return false;
+  I8Planes yp;
+  for (int s = 0; s < I8_S; ++s) yp.p[s] = g.yp[s];
+  if ((*st = slice_t(h, Y, N, 0, m, N, Rp, mx_of(h, 0), yp, exp_of(h, 0))) != RCHFSI_OK) return false;
+  g.active = true;
+  return true;
+}
+
+rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Z, int64_t ldz, int32_t w, int32_t zc0, double *H) {
+  I8GramState &g = h->i8g;
+  if (!g.active || w > g.max_w) { h->err = "gram_i8_slab: no planes"; return RCHFSI_EINVAL; }
+  const int64_t m = h->m;
+  I8Planes yp, zp;
+  for (int s = 0; s < I8_S; ++s) { yp.p[s] = g.yp[s]; zp.p[s] = g.zp[s]; }
+  const int32_t KS = choose_ks(h->N, w, zc0, m);
+  RCHFSI_TRY(ensure_hpart(h, sizeof(double) * (size_t)32 * h->N * g.max_w));
+  if (Z) {
+    RCHFSI_TRY(colmax(h, Z, ldz, w, mx_of(h, 1)));
+    RCHFSI_TRY(slice_t(h, Z, ldz, 0, m, w, g.Rp, mx_of(h, 1), zp, exp_of(h, 1)));
+  } else {                                                 // Y^T Y: the slab's own planes of Y
+    for (int s = 0; s < I8_S; ++s) zp.p[s] = g.yp[s] + (size_t)zc0 * g.Rp;
+  }
+  RCHFSI_TRY(gram_launch(h, yp, zp, g.Rp, m, w, zc0, false, KS));
+  return gram_finish(h, KS, w, zc0, exp_of(h, 0), Z ? exp_of(h, 1) : exp_of(h, 0) + zc0, H);
+}
+
+}  // namespace rchfsi
