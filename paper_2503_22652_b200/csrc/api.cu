@@ -86,6 +86,7 @@ static Knobs read_knobs() {
   k.rr_split = geti("RCHFSI_RR_SPLIT", -1);
   k.rr_i8_rows = geti("RCHFSI_RR_I8_ROWS", 0);
   k.rr_gram_i8 = geti("RCHFSI_RR_GRAM_I8", -1);
+  k.rr_i8_bn = geti("RCHFSI_RR_I8_BN", 128);
   k.host_chunk = geti("RCHFSI_HOST_CHUNK", 0);
 #ifdef RCHFSI_PROBES
   k.tc_debug = geti("RCHFSI_TC_DEBUG", 0);

@@ -60,6 +60,7 @@ struct Knobs {
   bool rr_timing = false;        // RCHFSI_RR_TIMING: print phase times of the Rayleigh-Ritz to stderr
   int rr_split = -1;             // RCHFSI_RR_SPLIT: rotation X = Y E on the INT8 tensor pipe (rr_i8.cu): 0 off, 1 forced, -1 = automatic
   int rr_gram_i8 = -1;           // RCHFSI_RR_GRAM_I8: Gram products Y^T (Op Y) on the INT8 tensor pipe: 0 off, 1 forced, -1 = automatic
+  int rr_i8_bn = 128;            // RCHFSI_RR_I8_BN: 128 = two-pass N_mma = 128 kernel (default), 64 = single-pass N_mma = 64 kernels
   int rr_i8_rows = 0;            // RCHFSI_RR_I8_ROWS: cap on the rows of one digit-plane chunk (tests: forces several chunks)
   int host_chunk = 0;            // RCHFSI_HOST_CHUNK: column-chunk width of rchfsi_filter_host (multiple of 128), 0 = automatic
   int tc_debug = 0;              // RCHFSI_TC_DEBUG (only in -DRCHFSI_PROBES builds)
@@ -350,6 +351,7 @@ size_t rr_i8_plan_bytes(int64_t m, int32_t N);   // digit planes of E, column ex
 rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, const double *BY, double *Ha, double *Hb,
                            void *scratch, size_t scratch_bytes);
 bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int32_t max_w, rchfsi_status *st);
-rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Z, int64_t ldz, int32_t w, int32_t zc0, double *H);
+rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Y, const double *Z1, const double *Z2, int64_t ldz, int32_t w, int32_t zc0,
+                           double *Ha, double *Hb);
 
 }  // namespace rchfsi

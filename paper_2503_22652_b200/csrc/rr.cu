@@ -271,7 +271,15 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     double budget = 6.0e9;
     if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) budget = std::max(budget, 0.33 * ((double)free_b - 12.0e9));   // 12 GB kept for the low-precision operator copies and scratch still to come
     int64_t cw = (int64_t)(budget / (16.0 * (double)m));
-    cw = std::max<int64_t>(8, std::min<int64_t>(N, cw >= 48 ? cw / 48 * 48 : cw / 8 * 8));   // multiples of the FE column tile
+    if (gram_i8_supported(h) && cw >= 64) {
+      // the INT8 Gram kernel takes the slabs of A Y_c and B Y_c side by side in 128-column tiles: keep 2 cw close to a
+      // multiple of 128
+      const int64_t w8 = cw / 8 * 8;
+      const double util = 2.0 * (double)w8 / (double)(cdiv(2 * w8, 128) * 128);
+      cw = std::min<int64_t>(N, util >= 0.85 ? w8 : cw / 64 * 64);
+    } else {
+      cw = std::max<int64_t>(8, std::min<int64_t>(N, cw >= 48 ? cw / 48 * 48 : cw / 8 * 8));   // multiples of the FE column tile
+    }
     h->rr_cw = (int32_t)cw;
     choose_row_panel(h);
   }
@@ -304,19 +312,17 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     const int32_t w = std::min(cw, N - c0);
     // lower triangle only (rows i >= c0 of this column slab): dsygvd reads nothing else
     RCHFSI_TRY(apply64(h, h->A.d, Y + c0, h->rrc1, w, N, w));
-    if (g8) RCHFSI_TRY(gram_i8_slab(h, h->rrc1, w, w, c0, h->Ha));
-    else CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc1, w, &zero,
-                                     h->Ha + (size_t)c0 * N + c0, N));
-    if (h->B.present) {
-      RCHFSI_TRY(apply64(h, h->B.d, Y + c0, h->rrc2, w, N, w));
-      if (g8) RCHFSI_TRY(gram_i8_slab(h, h->rrc2, w, w, c0, h->Hb));
-      else CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc2, w, &zero,
-                                       h->Hb + (size_t)c0 * N + c0, N));
-    } else {
-      if (g8) RCHFSI_TRY(gram_i8_slab(h, nullptr, 0, w, c0, h->Hb));
-      else CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, Y + c0, N, &zero,
-                                       h->Hb + (size_t)c0 * N + c0, N));
+    if (h->B.present) RCHFSI_TRY(apply64(h, h->B.d, Y + c0, h->rrc2, w, N, w));
+    if (g8) {
+      RCHFSI_TRY(gram_i8_slab(h, Y, h->rrc1, h->B.present ? h->rrc2 : nullptr, w, w, c0, h->Ha, h->Hb));
+      continue;
     }
+    const double *BYc = h->B.present ? h->rrc2 : Y + c0;
+    const int64_t ldb = h->B.present ? w : N;
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, h->rrc1, w, &zero,
+                                h->Ha + (size_t)c0 * N + c0, N));
+    CUBLAS_CHECK(h, cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_T, N - c0, w, (int)m, &one, Y + c0, N, BYc, (int)ldb, &zero,
+                                h->Hb + (size_t)c0 * N + c0, N));
     h->launches += 2;
   }
   h->i8g.active = false;

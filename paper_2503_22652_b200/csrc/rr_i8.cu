@@ -444,20 +444,260 @@ __global__ void __launch_bounds__(192, 1) i8_gram_kernel(const __grid_constant__
   if (warp == 2) tmem_dealloc(tmem_base, 512);
 }
 
-// H(a, zc0 + b) = 2^(ea_a + eb_b - 12) sum_ks Hpart[ks][b][a] for the lower triangle a >= zc0 + b (column-major H)
+// H(a, zc0 + b) = 2^(ea_a + eb_b - 12) sum_ks Hpart[ks][b][a] for the lower triangle a >= zc0 + b (column-major H).
+// w2 > 0: the Nz columns are two slabs of w2 columns side by side, the second one going to H2.
 __global__ void __launch_bounds__(256) i8_gram_finish_kernel(const double *__restrict__ Hpart, int32_t KS, int32_t N, int32_t Nz,
-                                                             int32_t zc0, const int32_t *__restrict__ ea,
-                                                             const int32_t *__restrict__ eb, double *__restrict__ H) {
+                                                             int32_t zc0, int32_t w2, const int32_t *__restrict__ ea,
+                                                             const int32_t *__restrict__ eb, double *__restrict__ H,
+                                                             double *__restrict__ H2) {
   const int b = blockIdx.y;
   const int eb_ = eb[b];
+  const int bb = (w2 > 0 && b >= w2) ? b - w2 : b;
+  double *Hd = (w2 > 0 && b >= w2) ? H2 : H;
   for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < N; a += gridDim.x * blockDim.x) {
-    if (a < zc0 + b) continue;
+    if (a < zc0 + bb) continue;
     double v = 0.0;
     for (int k = 0; k < KS; ++k) v += Hpart[((size_t)k * Nz + b) * N + a];
     const int ea_ = ea[a];
     const bool nan = ea_ == I8_NAN_ROW || eb_ == I8_NAN_ROW;
-    H[(size_t)(zc0 + b) * N + a] = nan ? __longlong_as_double(0x7ff8000000000000ll) : scalbn(v, ea_ + eb_ - 12);
+    Hd[(size_t)(zc0 + bb) * N + a] = nan ? __longlong_as_double(0x7ff8000000000000ll) : scalbn(v, ea_ + eb_ - 12);
   }
+}
+
+// ------------------------------------------------------------------------------------------------ N_mma = 128, two passes
+// The 128 x 64 x 32 MMA of the kernels above is operand-fetch bound (~80 cycles for 32 cycles of math).  With 128
+// output columns an MMA costs ~96 cycles for twice the work, but only 4 accumulators fit the 512 TMEM columns, so the
+// anti-diagonals are formed in two passes over K: pass 0 = d 0..3 (10 digit pairs), pass 1 = d 4..6 (18 pairs).  After
+// each pass the 8 epilogue warps drain the accumulators into FP64 registers (64 columns per thread; the passes and, for
+// the Gram products, the flush rounds add up there; one store at the end), and the MMA warp waits for the drain.  Inside a K block the planes are consumed as a sliding window:
+// for s = 0..dhi: acc[s+t-dlo] += A_s B_t^T for t = dhi-s .. max(dlo-s, 0); A_s and B_(dhi-s) are dead after step s, so
+// both operands stream through in-order rings (A ascending s, B descending t) of 6 x 16 KB each.
+constexpr int I8W_BN = 128;
+constexpr int I8W_TILE = 128 * 128;
+constexpr int I8W_SLOTS = 6;
+constexpr int I8W_SMEM = 2 * I8W_SLOTS * I8W_TILE + 1024 /*align*/ + 512 /*barriers*/;
+
+struct I8WParams {
+  int32_t MA, NB;          // valid extents of the M side (rows of the chunk / columns of Y) and of the N side
+  int32_t num_k_blocks;
+  // rotation (MODE 0)
+  double *Out;
+  int64_t ldo;
+  const int32_t *ea, *eb;
+  // Gram (MODE 1)
+  double *Hpart;           // [KS][NB][MA]
+  int32_t zc0;             // tiles with a0 + 127 < zc0 + (packed ? 0 : b0) are skipped
+  int32_t packed;          // N side = several column slabs side by side (all at global column zc0)
+  int32_t accumulate;      // the first drain adds to Hpart as well (row chunks after the first)
+};
+
+// one drain of the accumulators of a pass into the thread's FP64 registers: NACC = 4 (anti-diagonals 0..3) or 3 (4..6,
+// weight 2^-32); the thread owns TMEM lane 32 qd + lane and the 64 columns of its half
+template <int NACC>
+__device__ __forceinline__ void i8w_drain(double (&acc)[64], uint32_t tmem_base, int qd, int half) {
+#pragma unroll
+  for (int c0 = 0; c0 < 64; c0 += 8) {
+    uint32_t v[NACC][8];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i)
+      tmem_ld_32x8(tmem_base + ((uint32_t)(32 * qd) << 16) + (uint32_t)(i * I8W_BN + half * 64 + c0), v[i]);
+    tmem_ld_wait();
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      double x = (double)(int32_t)v[NACC - 1][u];
+#pragma unroll
+      for (int i = NACC - 2; i >= 0; --i) x = fma(x, 0.00390625, (double)(int32_t)v[i][u]);
+      acc[c0 + u] = (NACC == 3) ? fma(x, 2.3283064365386963e-10, acc[c0 + u]) : acc[c0 + u] + x;   // 2^-32
+    }
+  }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(320, 1) i8w_kernel(const __grid_constant__ I8Maps mapsA, const __grid_constant__ I8Maps mapsB,
+                                                     I8WParams p) {
+  const int b0 = blockIdx.x * I8W_BN;
+  const int a0 = blockIdx.y * 128;
+  if (MODE == 1 && a0 + 127 < p.zc0 + (p.packed ? 0 : b0)) return;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t *As = smem;
+  uint8_t *Bs = smem + I8W_SLOTS * I8W_TILE;
+  uint64_t *a_full = reinterpret_cast<uint64_t *>(Bs + I8W_SLOTS * I8W_TILE);
+  uint64_t *a_empty = a_full + I8W_SLOTS;
+  uint64_t *b_full = a_empty + I8W_SLOTS;
+  uint64_t *b_empty = b_full + I8W_SLOTS;
+  uint64_t *accum_bar = b_empty + I8W_SLOTS;
+  uint64_t *drained_bar = accum_bar + 1;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(drained_bar + 1);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int ks = gridDim.z;
+  const int kb0 = (int)((int64_t)p.num_k_blocks * blockIdx.z / ks);
+  const int nk = (int)((int64_t)p.num_k_blocks * (blockIdx.z + 1) / ks) - kb0;
+  const int round_len = MODE == 1 ? I8_FLUSH : nk;                   // K blocks between two drains of one pass
+  const int rounds = nk > 0 ? (nk + round_len - 1) / round_len : 0;
+
+  if (warp == 0 && lane == 0) {
+    for (int s = 0; s < I8_S; ++s) {
+      tma_prefetch_desc(&mapsA.m[s]);
+      tma_prefetch_desc(&mapsB.m[s]);
+    }
+    for (int s = 0; s < I8W_SLOTS; ++s) {
+      mbar_init(a_full + s, 1);
+      mbar_init(a_empty + s, 1);
+      mbar_init(b_full + s, 1);
+      mbar_init(b_empty + s, 1);
+    }
+    mbar_init(accum_bar, 1);
+    mbar_init(drained_bar, 8);
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===== TMA producer: tiles in the order the MMA loop first needs them
+    int it = 0;                                  // tiles issued so far on each ring (both rings advance together)
+    for (int rd = 0; rd < rounds; ++rd) {
+      const int c_lo = rd * round_len, c_hi = min(nk, c_lo + round_len);
+      for (int pass = 0; pass < 2; ++pass) {
+        const int dlo = pass ? 4 : 0, dhi = pass ? 6 : 3;
+        for (int c = c_lo; c < c_hi; ++c) {
+          const int k0 = (kb0 + c) * 128;
+          for (int s = 0; s <= dhi; ++s) {
+            // B planes first needed at step s: t = dhi .. dlo at s = 0, t = dlo - s afterwards; ring position dhi - t
+            const int t_first = s == 0 ? dhi : dlo - s, t_last = s == 0 ? dlo : dlo - s;
+            for (int t = t_first; t >= t_last && t >= 0; --t) {
+              const int ib = it + (dhi - t);
+              const int slot = ib % I8W_SLOTS;
+              mbar_wait(b_empty + slot, ((ib / I8W_SLOTS) & 1) ^ 1);
+              if (elect_one()) {
+                mbar_expect_tx(b_full + slot, I8W_TILE);
+                tma_load_2d(Bs + slot * I8W_TILE, &mapsB.m[t], b_full + slot, k0, b0);
+              }
+              __syncwarp();
+            }
+            const int ia = it + s;
+            const int slot = ia % I8W_SLOTS;
+            mbar_wait(a_empty + slot, ((ia / I8W_SLOTS) & 1) ^ 1);
+            if (elect_one()) {
+              mbar_expect_tx(a_full + slot, I8W_TILE);
+              tma_load_2d(As + slot * I8W_TILE, &mapsA.m[s], a_full + slot, k0, a0);
+            }
+            __syncwarp();
+          }
+          it += dhi + 1;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer
+    constexpr uint32_t idesc = make_idesc_i8(128, I8W_BN);
+    const uint64_t da0 = make_smem_desc(smem_u32(As), 16, 1024, 2);
+    const uint64_t db0 = make_smem_desc(smem_u32(Bs), 16, 1024, 2);
+    int it = 0, drains = 0;
+    for (int rd = 0; rd < rounds; ++rd) {
+      const int c_lo = rd * round_len, c_hi = min(nk, c_lo + round_len);
+      for (int pass = 0; pass < 2; ++pass) {
+        const int dlo = pass ? 4 : 0, dhi = pass ? 6 : 3;
+        if (drains > 0) {                        // the epilogue has read the accumulators of the previous pass
+          mbar_wait(drained_bar, (drains - 1) & 1);
+          tc_fence_after();
+        }
+        for (int c = c_lo; c < c_hi; ++c) {
+          for (int s = 0; s <= dhi; ++s) {
+            const int t_first = s == 0 ? dhi : dlo - s, t_last = s == 0 ? dlo : dlo - s;
+            for (int t = t_first; t >= t_last && t >= 0; --t) {
+              const int ib = it + (dhi - t);
+              mbar_wait(b_full + ib % I8W_SLOTS, (ib / I8W_SLOTS) & 1);
+            }
+            const int ia = it + s;
+            mbar_wait(a_full + ia % I8W_SLOTS, (ia / I8W_SLOTS) & 1);
+            tc_fence_after();
+            if (elect_one()) {
+              const uint64_t da = da0 + (uint32_t)(((ia % I8W_SLOTS) * I8W_TILE) >> 4);
+              const int t_hi = dhi - s, t_lo = dlo - s > 0 ? dlo - s : 0;
+              for (int t = t_hi; t >= t_lo; --t) {
+                const int ib = it + (dhi - t);
+                const uint64_t db = db0 + (uint32_t)(((ib % I8W_SLOTS) * I8W_TILE) >> 4);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                  umma_i8(tmem_base + (uint32_t)((s + t - dlo) * I8W_BN), da + 2 * q, db + 2 * q, idesc,
+                          (c > c_lo || s > 0 || q > 0) ? 1u : 0u);
+              }
+              umma_commit(a_empty + ia % I8W_SLOTS);
+              umma_commit(b_empty + (it + s) % I8W_SLOTS);          // plane dhi - s: its last use
+              if (s == dhi && c == c_hi - 1) umma_commit(accum_bar);
+            }
+            __syncwarp();
+          }
+          it += dhi + 1;
+        }
+        ++drains;
+      }
+    }
+  } else {
+    // ===== epilogue (8 warps): thread = accumulator row (TMEM lane 32 (warp % 4) + lane) x one 64-column half; the
+    // passes (and, for the Gram products, the flush rounds) add up in FP64 registers, one store at the end
+    const int qd = warp & 3;
+    const int half = (warp - 2) >> 2;
+    const int a = a0 + 32 * qd + lane;
+    const bool aok = a < p.MA;
+    double acc[64];
+#pragma unroll
+    for (int u = 0; u < 64; ++u) acc[u] = 0.0;
+    int drains = 0;
+    for (int rd = 0; rd < rounds; ++rd) {
+      for (int pass = 0; pass < 2; ++pass) {
+        mbar_wait(accum_bar, drains & 1);
+        tc_fence_after();
+        if (pass == 0) i8w_drain<4>(acc, tmem_base, qd, half);
+        else i8w_drain<3>(acc, tmem_base, qd, half);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(drained_bar);
+        ++drains;
+      }
+    }
+    const int bh = b0 + half * 64;
+    if (aok) {
+      if (MODE == 0) {
+        const int ea = p.ea[a];
+        double *__restrict__ orow = p.Out + (int64_t)a * p.ldo;
+#pragma unroll
+        for (int c0 = 0; c0 < 64; c0 += 8) {
+          int eb[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) eb[u] = (bh + c0 + u < p.NB) ? __ldg(p.eb + bh + c0 + u) : 0;
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const int b = bh + c0 + u;
+            if (b < p.NB)
+              orow[b] = (ea == I8_NAN_ROW || eb[u] == I8_NAN_ROW) ? __longlong_as_double(0x7ff8000000000000ll)
+                                                                  : scalbn(acc[c0 + u], ea + eb[u] - 12);
+          }
+        }
+      } else {
+        double *__restrict__ hp = p.Hpart + ((size_t)blockIdx.z * p.NB) * p.MA + a;
+#pragma unroll
+        for (int c0 = 0; c0 < 64; c0 += 8) {
+          double old[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) old[u] = (p.accumulate && bh + c0 + u < p.NB) ? hp[(size_t)(bh + c0 + u) * p.MA] : 0.0;
+#pragma unroll
+          for (int u = 0; u < 8; ++u)
+            if (bh + c0 + u < p.NB) hp[(size_t)(bh + c0 + u) * p.MA] = old[u] + acc[c0 + u];
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tmem_base, 512);
 }
 
 }  // namespace
@@ -465,7 +705,7 @@ __global__ void __launch_bounds__(256) i8_gram_finish_kernel(const double *__res
 bool rotate_i8_supported(const rchfsi_ctx *h) {
   if (h->knobs.rr_split == 0) return false;
   if (h->N > 16384) return false;                         // INT32 exactness: 7 N 2^14 < 2^31
-  if (h->knobs.rr_split > 0) return h->N >= 16;              // forced (tests at small sizes)
+  if (h->knobs.rr_split > 0) return h->N >= 16;           // forced (tests at small sizes)
   return h->N >= 256 && h->m >= 8192;                     // where it beats dgemm
 }
 
@@ -473,6 +713,18 @@ size_t rotate_i8_fixed_bytes(int32_t N) {
   const size_t Kp = ((size_t)N + 15) / 16 * 16;
   return (size_t)I8_S * N * Kp + 4 * (size_t)N + 1024;
 }
+
+namespace {
+
+bool wide(const rchfsi_ctx *h) { return h->knobs.rr_i8_bn != 64; }   // N_mma = 128 two-pass kernel (default) or 64
+
+bool plane_maps(rchfsi_ctx *h, I8Maps *maps, const I8Planes &pl, int64_t rows, int64_t K, uint32_t box_rows) {
+  for (int s = 0; s < I8_S; ++s)
+    if (!get_tmap_2d(h, &maps->m[s], pl.p[s], 1, false, (uint64_t)rows, (uint64_t)K, (uint64_t)K, 128, box_rows)) return false;
+  return true;
+}
+
+}  // namespace
 
 // Out[r][:] = In[r][:] E for r < rows (E column-major N x N); Out may be In.  `scratch` holds the digit planes and
 // exponents of one row chunk: the more rows fit, the fewer chunk launches.
@@ -488,15 +740,38 @@ rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const dou
   R = std::min<int64_t>(R, rows);
   if (h->knobs.rr_i8_rows > 0) R = std::min<int64_t>(R, h->knobs.rr_i8_rows);
   if (R >= 128) R = R / 128 * 128;
-  if (R < 1 || R > 0x7fffff00 / I8_S) R = std::min<int64_t>(R, 0x7fffff00 / I8_S);
+  R = std::min<int64_t>(R, 0x7fffff00 / I8_S);
   if (R < 1) { h->err = "rotate_i8: scratch too small"; return RCHFSI_EINVAL; }
   int8_t *Aplanes = reinterpret_cast<int8_t *>(scratch);
   int32_t *ea = reinterpret_cast<int32_t *>(Aplanes + ((size_t)I8_S * R * Kp + 255) / 256 * 256);
-  RCHFSI_TRY(ensure_func_smem(h, (const void *)i8_rotate_kernel, I8_SMEM));
   cudaStream_t st = h->stream;
   // digit planes of the columns of E (column-major: column j is contiguous, i.e. a "row" of the slicing kernel)
   i8_slice_kernel<<<(unsigned)cdiv(N, 8), 256, 0, st>>>(E, N, N, N, Kp, Eplanes, N, eb);
   LAUNCH_CHECK(h);
+  if (wide(h)) {
+    RCHFSI_TRY(ensure_func_smem(h, (const void *)i8w_kernel<0>, I8W_SMEM));
+    I8Planes pe;
+    for (int s = 0; s < I8_S; ++s) pe.p[s] = Eplanes + (size_t)s * N * Kp;
+    I8Maps mb;
+    if (!plane_maps(h, &mb, pe, N, Kp, 128)) { h->err = "rotate_i8: cuTensorMapEncodeTiled failed (E planes)"; return RCHFSI_ECUDA; }
+    for (int64_t r0 = 0; r0 < rows; r0 += R) {
+      const int64_t rc = std::min<int64_t>(R, rows - r0);
+      i8_slice_kernel<<<(unsigned)cdiv(rc, 8), 256, 0, st>>>(In + (size_t)r0 * N, N, rc, N, Kp, Aplanes, rc, ea);
+      LAUNCH_CHECK(h);
+      I8Planes pa;
+      for (int s = 0; s < I8_S; ++s) pa.p[s] = Aplanes + (size_t)s * rc * Kp;
+      I8Maps ma;
+      if (!plane_maps(h, &ma, pa, rc, Kp, 128)) { h->err = "rotate_i8: cuTensorMapEncodeTiled failed (Y planes)"; return RCHFSI_ECUDA; }
+      I8WParams p{};
+      p.MA = (int32_t)rc; p.NB = N; p.num_k_blocks = (int32_t)cdiv(N, 128);
+      p.Out = Out + (size_t)r0 * N; p.ldo = N; p.ea = ea; p.eb = eb;
+      dim3 grid((unsigned)cdiv(N, I8W_BN), (unsigned)cdiv(rc, 128), 1);
+      i8w_kernel<0><<<grid, 320, I8W_SMEM, st>>>(ma, mb, p);
+      LAUNCH_CHECK(h);
+    }
+    return RCHFSI_OK;
+  }
+  RCHFSI_TRY(ensure_func_smem(h, (const void *)i8_rotate_kernel, I8_SMEM));
   CUtensorMap tmB;
   if (!get_tmap_2d(h, &tmB, Eplanes, 1, false, (uint64_t)I8_S * N, (uint64_t)Kp, (uint64_t)Kp, 128, I8_BN)) {
     h->err = "rotate_i8: cuTensorMapEncodeTiled failed (E planes)";
@@ -541,12 +816,13 @@ bool carve(std::vector<I8Buf> &bufs, size_t bytes, void **out) {
   return false;
 }
 
-rchfsi_status i8_fixed(rchfsi_ctx *h) {   // column maxima and exponents of Y and Z
-  if (!h->i8_cols) RCHFSI_TRY(dev_alloc(h, &h->i8_cols, (size_t)h->N_cap * 24 + 1024));
+// column maxima (bit patterns) and exponents: Y [N], Z [2 N] (two slabs side by side)
+rchfsi_status i8_fixed(rchfsi_ctx *h) {
+  if (!h->i8_cols) RCHFSI_TRY(dev_alloc(h, &h->i8_cols, (size_t)h->N_cap * 36 + 1024));
   return RCHFSI_OK;
 }
 unsigned long long *mx_of(rchfsi_ctx *h, int which) { return reinterpret_cast<unsigned long long *>(h->i8_cols) + (size_t)which * h->N_cap; }
-int32_t *exp_of(rchfsi_ctx *h, int which) { return reinterpret_cast<int32_t *>(mx_of(h, 2)) + (size_t)which * h->N_cap; }
+int32_t *exp_of(rchfsi_ctx *h, int which) { return reinterpret_cast<int32_t *>(mx_of(h, 3)) + (size_t)which * h->N_cap; }
 
 rchfsi_status colmax(rchfsi_ctx *h, const double *V, int64_t ld, int32_t cols, unsigned long long *mx) {
   RCHFSI_CUDA_CHECK(h, cudaMemsetAsync(mx, 0, sizeof(unsigned long long) * cols, h->stream));
@@ -566,35 +842,48 @@ rchfsi_status slice_t(rchfsi_ctx *h, const double *V, int64_t ld, int64_t r0, in
   return RCHFSI_OK;
 }
 
-bool plane_maps(rchfsi_ctx *h, I8Maps *maps, const I8Planes &pl, int32_t cols, int64_t Rp, uint32_t box_rows) {
-  for (int s = 0; s < I8_S; ++s)
-    if (!get_tmap_2d(h, &maps->m[s], pl.p[s], 1, false, (uint64_t)cols, (uint64_t)Rp, (uint64_t)Rp, 128, box_rows)) return false;
-  return true;
+I8Planes shifted(const I8Planes &pl, size_t bytes) {
+  I8Planes o;
+  for (int s = 0; s < I8_S; ++s) o.p[s] = pl.p[s] + bytes;
+  return o;
 }
 
-// one slab: Hpart (+)= Y^T Z over the K blocks of this row chunk, then (last chunk) H = scaled sum
+int32_t choose_ks(const rchfsi_ctx *h, int32_t N, int32_t Nz, int32_t zc0, bool packed, int64_t rows) {
+  const int bn = wide(h) ? I8W_BN : I8_BN;
+  int64_t tiles = 0;
+  for (int a0 = 0; a0 < N; a0 += 128)
+    for (int b0 = 0; b0 < Nz; b0 += bn) tiles += (a0 + 127 >= zc0 + (packed ? 0 : b0));
+  const int64_t nkb = cdiv(rows, 128);
+  const int64_t ks = ((int64_t)4 * 148) / std::max<int64_t>(tiles, 1);      // at most 4 full waves of CTAs (one per SM)
+  return (int32_t)std::max<int64_t>(1, std::min<int64_t>({ks, (int64_t)32, nkb}));
+}
+
+// Hpart (+)= Y^T Z over the K blocks of this row chunk
 rchfsi_status gram_launch(rchfsi_ctx *h, const I8Planes &yp, const I8Planes &zp, int64_t Rp, int64_t rows, int32_t Nz, int32_t zc0,
-                          bool accumulate, int32_t KS) {
+                          bool packed, bool accumulate, int32_t KS) {
   I8Maps ma, mb;
-  if (!plane_maps(h, &ma, yp, h->N, Rp, 128) || !plane_maps(h, &mb, zp, Nz, Rp, I8_BN)) {
+  const bool w = wide(h);
+  if (!plane_maps(h, &ma, yp, h->N, Rp, 128) || !plane_maps(h, &mb, zp, Nz, Rp, w ? 128 : I8_BN)) {
     h->err = "gram_i8: cuTensorMapEncodeTiled failed";
     return RCHFSI_ECUDA;
   }
+  if (w) {
+    RCHFSI_TRY(ensure_func_smem(h, (const void *)i8w_kernel<1>, I8W_SMEM));
+    I8WParams p{};
+    p.MA = h->N; p.NB = Nz; p.num_k_blocks = (int32_t)cdiv(rows, 128);
+    p.Hpart = reinterpret_cast<double *>(h->i8_hpart); p.zc0 = zc0; p.packed = packed ? 1 : 0; p.accumulate = accumulate ? 1 : 0;
+    dim3 grid((unsigned)cdiv(Nz, I8W_BN), (unsigned)cdiv(h->N, 128), (unsigned)KS);
+    i8w_kernel<1><<<grid, 320, I8W_SMEM, h->stream>>>(ma, mb, p);
+    LAUNCH_CHECK(h);
+    return RCHFSI_OK;
+  }
+  if (packed) { h->err = "gram_i8: the 64-column kernel takes one slab at a time"; return RCHFSI_EINVAL; }
   RCHFSI_TRY(ensure_func_smem(h, (const void *)i8_gram_kernel, I8_SMEM));
   I8GramParams p{reinterpret_cast<double *>(h->i8_hpart), h->N, Nz, zc0, (int32_t)cdiv(rows, 128), accumulate ? 1 : 0};
   dim3 grid((unsigned)cdiv(Nz, I8_BN), (unsigned)cdiv(h->N, 128), (unsigned)KS);
   i8_gram_kernel<<<grid, 192, I8_SMEM, h->stream>>>(ma, mb, p);
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
-}
-
-int32_t choose_ks(int32_t N, int32_t Nz, int32_t zc0, int64_t rows) {
-  int64_t tiles = 0;
-  for (int a0 = 0; a0 < N; a0 += 128)
-    for (int b0 = 0; b0 < Nz; b0 += I8_BN) tiles += (a0 + 127 >= zc0 + b0);
-  const int64_t nkb = cdiv(rows, 128);
-  int64_t ks = cdiv((int64_t)4 * 148, std::max<int64_t>(tiles, 1));
-  return (int32_t)std::max<int64_t>(1, std::min<int64_t>({ks, (int64_t)32, nkb}));
 }
 
 rchfsi_status ensure_hpart(rchfsi_ctx *h, size_t bytes) {
@@ -605,9 +894,10 @@ rchfsi_status ensure_hpart(rchfsi_ctx *h, size_t bytes) {
   return RCHFSI_OK;
 }
 
-rchfsi_status gram_finish(rchfsi_ctx *h, int32_t KS, int32_t Nz, int32_t zc0, const int32_t *ea, const int32_t *eb, double *H) {
+rchfsi_status gram_finish(rchfsi_ctx *h, int32_t KS, int32_t Nz, int32_t zc0, int32_t w2, const int32_t *ea, const int32_t *eb,
+                          double *H, double *H2) {
   dim3 grid((unsigned)cdiv(h->N, 256), (unsigned)Nz);
-  i8_gram_finish_kernel<<<grid, 256, 0, h->stream>>>(reinterpret_cast<const double *>(h->i8_hpart), KS, h->N, Nz, zc0, ea, eb, H);
+  i8_gram_finish_kernel<<<grid, 256, 0, h->stream>>>(reinterpret_cast<const double *>(h->i8_hpart), KS, h->N, Nz, zc0, w2, ea, eb, H, H2);
   LAUNCH_CHECK(h);
   return RCHFSI_OK;
 }
@@ -618,7 +908,11 @@ rchfsi_status gram_finish(rchfsi_ctx *h, int32_t KS, int32_t Nz, int32_t zc0, co
 size_t rr_i8_plan_bytes(int64_t m, int32_t N) {
   if (N < 256 || m < 8192 || N > 16384) return 0;
   auto al = [](size_t b) { return (b + 255) / 256 * 256; };
-  return al(rotate_i8_fixed_bytes(N)) + al((size_t)N * 24 + 1024) + al(sizeof(double) * (size_t)choose_ks(N, N, 0, m) * N * N);
+  int64_t tiles = 0;
+  for (int a0 = 0; a0 < N; a0 += 128)
+    for (int b0 = 0; b0 < N; b0 += I8W_BN) tiles += (a0 + 127 >= b0);
+  const int64_t ks = std::max<int64_t>(1, std::min<int64_t>({((int64_t)4 * 148) / std::max<int64_t>(tiles, 1), (int64_t)32, cdiv(m, 128)}));
+  return al(rotate_i8_fixed_bytes(N)) + al((size_t)N * 36 + 1024) + al(sizeof(double) * (size_t)ks * N * N);
 }
 
 // Full-block variant: H_a = Y^T (AY), H_b = Y^T (BY) (BY == NULL: Y^T Y), lower triangles, column-major.  `scratch`
@@ -641,7 +935,7 @@ rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, con
     yp.p[s] = reinterpret_cast<int8_t *>(base + (size_t)s * N * Rp);
     zp.p[s] = reinterpret_cast<int8_t *>(base + (size_t)(I8_S + s) * N * Rp);
   }
-  const int32_t KS = choose_ks(N, N, 0, R);
+  const int32_t KS = choose_ks(h, N, N, 0, false, R);
   RCHFSI_TRY(ensure_hpart(h, sizeof(double) * (size_t)KS * N * N));
   RCHFSI_TRY(colmax(h, Y, N, N, mx_of(h, 0)));
   for (int prod = 0; prod < 2; ++prod) {
@@ -652,16 +946,17 @@ rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, con
       const int64_t rc = std::min<int64_t>(R, m - r0);
       RCHFSI_TRY(slice_t(h, Y, N, r0, rc, N, Rp, mx_of(h, 0), yp, exp_of(h, 0)));
       if (!same) RCHFSI_TRY(slice_t(h, Z, N, r0, rc, N, Rp, mx_of(h, 1), zp, exp_of(h, 1)));
-      RCHFSI_TRY(gram_launch(h, yp, same ? yp : zp, Rp, rc, N, 0, r0 > 0, KS));
+      RCHFSI_TRY(gram_launch(h, yp, same ? yp : zp, Rp, rc, N, 0, false, r0 > 0, KS));
     }
-    RCHFSI_TRY(gram_finish(h, KS, N, 0, exp_of(h, 0), same ? exp_of(h, 0) : exp_of(h, 1), prod == 0 ? Ha : Hb));
+    RCHFSI_TRY(gram_finish(h, KS, N, 0, 0, exp_of(h, 0), same ? exp_of(h, 0) : exp_of(h, 1), prod == 0 ? Ha : Hb, nullptr));
   }
   return RCHFSI_OK;
 }
 
 // Column-slab variant (memory-light Rayleigh-Ritz): the transposed planes of ALL rows of Y are built once into the
-// caller's buffers (the filter's dead blocks), then every column slab Z_c = Op Y[:, c0:c0+w] contributes
-// H[:, c0:c0+w] = Y^T Z_c.  Returns false (nothing launched) when the buffers cannot hold the planes.
+// caller's buffers (the filter's dead blocks), then every column slab contributes H_a[:, c0:c0+w] = Y^T (A Y_c) and
+// H_b[:, c0:c0+w] = Y^T (B Y_c) in ONE launch (the two slabs side by side on the N side: Y's planes are read once).
+// Returns false (nothing launched) when the buffers cannot hold the planes.
 bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int32_t max_w, rchfsi_status *st) {
   *st = RCHFSI_OK;
   const int32_t N = h->N;
@@ -672,10 +967,11 @@ bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int3
   for (int s = 0; s < I8_S; ++s)
     if (!carve(bufs, (size_t)N * Rp, reinterpret_cast<void **>(&g.yp[s]))) return false;
   for (int s = 0; s < I8_S; ++s)
-    if (!carve(bufs, (size_t)max_w * Rp, reinterpret_cast<void **>(&g.zp[s]))) return false;
+    if (!carve(bufs, (size_t)2 * max_w * Rp, reinterpret_cast<void **>(&g.zp[s]))) return false;
   g.Rp = Rp;
   g.max_w = max_w;
   if ((*st = i8_fixed(h)) != RCHFSI_OK) return false;
+  if ((*st = ensure_hpart(h, sizeof(double) * (size_t)32 * N * 2 * max_w)) != RCHFSI_OK) return false;
   if ((*st = colmax(h, Y, N, N, mx_of(h, 0))) != RCHFSI_OK) return false;
   I8Planes yp;
   for (int s = 0; s < I8_S; ++s) yp.p[s] = g.yp[s];
@@ -684,22 +980,31 @@ bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int3
   return true;
 }
 
-rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Z, int64_t ldz, int32_t w, int32_t zc0, double *H) {
+// Z1 = A Y_c, Z2 = B Y_c ([m][w], pitch ldz) or NULL for B = I (the slab of Y itself)
+rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Y, const double *Z1, const double *Z2, int64_t ldz, int32_t w, int32_t zc0,
+                           double *Ha, double *Hb) {
   I8GramState &g = h->i8g;
   if (!g.active || w > g.max_w) { h->err = "gram_i8_slab: no planes"; return RCHFSI_EINVAL; }
   const int64_t m = h->m;
   I8Planes yp, zp;
   for (int s = 0; s < I8_S; ++s) { yp.p[s] = g.yp[s]; zp.p[s] = g.zp[s]; }
-  const int32_t KS = choose_ks(h->N, w, zc0, m);
-  RCHFSI_TRY(ensure_hpart(h, sizeof(double) * (size_t)32 * h->N * g.max_w));
-  if (Z) {
-    RCHFSI_TRY(colmax(h, Z, ldz, w, mx_of(h, 1)));
-    RCHFSI_TRY(slice_t(h, Z, ldz, 0, m, w, g.Rp, mx_of(h, 1), zp, exp_of(h, 1)));
-  } else {                                                 // Y^T Y: the slab's own planes of Y
-    for (int s = 0; s < I8_S; ++s) zp.p[s] = g.yp[s] + (size_t)zc0 * g.Rp;
+  RCHFSI_TRY(colmax(h, Z1, ldz, w, mx_of(h, 1)));
+  RCHFSI_TRY(slice_t(h, Z1, ldz, 0, m, w, g.Rp, mx_of(h, 1), zp, exp_of(h, 1)));
+  const double *Zb = Z2 ? Z2 : Y + zc0;
+  const int64_t ldb = Z2 ? ldz : h->N;
+  RCHFSI_TRY(colmax(h, Zb, ldb, w, mx_of(h, 1) + w));
+  RCHFSI_TRY(slice_t(h, Zb, ldb, 0, m, w, g.Rp, mx_of(h, 1) + w, shifted(zp, (size_t)w * g.Rp), exp_of(h, 1) + w));
+  if (wide(h)) {
+    const int32_t KS = choose_ks(h, h->N, 2 * w, zc0, true, m);
+    RCHFSI_TRY(gram_launch(h, yp, zp, g.Rp, m, 2 * w, zc0, true, false, KS));
+    return gram_finish(h, KS, 2 * w, zc0, w, exp_of(h, 0), exp_of(h, 1), Ha, Hb);
   }
-  RCHFSI_TRY(gram_launch(h, yp, zp, g.Rp, m, w, zc0, false, KS));
-  return gram_finish(h, KS, w, zc0, exp_of(h, 0), Z ? exp_of(h, 1) : exp_of(h, 0) + zc0, H);
+  for (int prod = 0; prod < 2; ++prod) {                  // 64-column kernel: one slab per launch
+    const int32_t KS = choose_ks(h, h->N, w, zc0, false, m);
+    RCHFSI_TRY(gram_launch(h, yp, prod ? shifted(zp, (size_t)w * g.Rp) : zp, g.Rp, m, w, zc0, false, false, KS));
+    RCHFSI_TRY(gram_finish(h, KS, w, zc0, 0, exp_of(h, 0), exp_of(h, 1) + prod * w, prod ? Hb : Ha, nullptr));
+  }
+  return RCHFSI_OK;
 }
 
 }  // namespace rchfsi

@@ -11,9 +11,10 @@ from tests.helpers import oracle_ops, small_dense_generalized
 pytestmark = pytest.mark.gpu
 
 
-def _rr(prob, Y, monkeypatch, split, chunked="0", rows=None, gram="0", prefilter=False):
+def _rr(prob, Y, monkeypatch, split, chunked="0", rows=None, gram="0", prefilter=False, bn="128"):
     import torch
     import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_RR_I8_BN", bn)
     monkeypatch.setenv("RCHFSI_RR_SPLIT", split)
     monkeypatch.setenv("RCHFSI_RR_GRAM_I8", gram)
     monkeypatch.setenv("RCHFSI_RR_CHUNKED", chunked)
@@ -35,15 +36,16 @@ def _rr(prob, Y, monkeypatch, split, chunked="0", rows=None, gram="0", prefilter
     return out + (launches,)
 
 
+@pytest.mark.parametrize("bn", ["128", "64"])
 @pytest.mark.parametrize("m,N,chunked,rows", [(700, 300, "0", None), (700, 300, "1", 256), (1000, 137, "0", 384),
                                               (333, 64, "1", None)])
-def test_int8_rotation_matches_oracle_and_dgemm_path(monkeypatch, m, N, chunked, rows):
+def test_int8_rotation_matches_oracle_and_dgemm_path(monkeypatch, m, N, chunked, rows, bn):
     prob = small_dense_generalized(m, seed=3)
     A, B, _ = oracle_ops(prob)
     Y = np.random.default_rng(8).standard_normal((m, N)) * np.logspace(0, 6, N)[None, :]
     ritz_o, X_o, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, Y)
     res_o = orc.residual_norms(AX, BX, ritz_o)
-    ritz, X, G, res, _ = _rr(prob, Y, monkeypatch, "1", chunked, rows)
+    ritz, X, G, res, _ = _rr(prob, Y, monkeypatch, "1", chunked, rows, bn=bn)
     ritz_d, X_d, G_d, res_d, _ = _rr(prob, Y, monkeypatch, "0", chunked)
     Bd = prob["B"]
     np.testing.assert_allclose(ritz, ritz_o, rtol=1e-11, atol=1e-12)
@@ -58,10 +60,11 @@ def test_int8_rotation_matches_oracle_and_dgemm_path(monkeypatch, m, N, chunked,
     np.testing.assert_allclose(res, res_d, rtol=1e-6, atol=1e-11)
 
 
-def _rotate(Y, E, monkeypatch, split, rows=None):
+def _rotate(Y, E, monkeypatch, split, rows=None, bn="128"):
     """rchfsi_rotate on a handle of a throw-away operator (the rotation does not touch the operator)."""
     import torch
     import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_RR_I8_BN", bn)
     monkeypatch.setenv("RCHFSI_RR_SPLIT", split)
     if rows:
         monkeypatch.setenv("RCHFSI_RR_I8_ROWS", str(rows))
@@ -79,8 +82,9 @@ def _rotate(Y, E, monkeypatch, split, rows=None):
     return out
 
 
-@pytest.mark.parametrize("m,N,rows", [(900, 260, None), (1500, 129, 512), (2500, 2400, 1024), (130, 16, None)])
-def test_int8_rotation_error_is_at_the_fp64_level_for_badly_scaled_operands(monkeypatch, m, N, rows):
+@pytest.mark.parametrize("m,N,rows,bn", [(900, 260, None, "128"), (1500, 129, 512, "128"), (2500, 2400, 1024, "128"),
+                                         (130, 16, None, "128"), (900, 260, None, "64"), (2500, 2400, 1024, "64")])
+def test_int8_rotation_error_is_at_the_fp64_level_for_badly_scaled_operands(monkeypatch, m, N, rows, bn):
     """Entries spanning 12 orders of magnitude inside a row of Y, rows of Y and columns of E differing by 2^+-100 in
     scale, an all-zero row: against a longdouble product (sampled rows) the INT8 result is within 8 sqrt(K) FP64 ulps of
     (row max of Y)(column max of E) per element -- the norm the fixed-point split is exact in; the dgemm path's own
@@ -91,7 +95,7 @@ def test_int8_rotation_error_is_at_the_fp64_level_for_badly_scaled_operands(monk
     Y[5, :] = 0.0
     E = np.linalg.qr(rng.standard_normal((N, N)))[0] * 10.0 ** rng.uniform(-3, 0, (N, N))
     E *= 2.0 ** rng.integers(-100, 100, (1, N))
-    X1 = _rotate(Y, E, monkeypatch, "1", rows)
+    X1 = _rotate(Y, E, monkeypatch, "1", rows, bn)
     X0 = _rotate(Y, E, monkeypatch, "0")
     rs = np.unique(np.concatenate(([0, 5, 127, 128, m - 1], rng.integers(0, m, 59))))
     ref = Y[rs].astype(np.longdouble) @ E.astype(np.longdouble)
@@ -104,7 +108,7 @@ def test_int8_rotation_error_is_at_the_fp64_level_for_badly_scaled_operands(monk
     assert np.all(np.abs(X1 - X0) <= 1e-12 * full)                        # every element, against the dgemm path
     assert np.all(X1[5] == 0.0)
     # power-of-two row scaling commutes with the product exactly (row exponents)
-    X2 = _rotate(Y * 2.0 ** 37, E, monkeypatch, "1", rows)
+    X2 = _rotate(Y * 2.0 ** 37, E, monkeypatch, "1", rows, bn)
     assert np.array_equal(X2, X1 * 2.0 ** 37)
 
 
@@ -121,10 +125,11 @@ def test_int8_rotation_propagates_non_finite_rows(monkeypatch):
     np.testing.assert_allclose(X[ok], Y[ok] @ E, rtol=0, atol=1e-13)
 
 
+@pytest.mark.parametrize("bn", ["128", "64"])
 @pytest.mark.parametrize("m,N,chunked,rows,generalized", [(700, 300, "0", None, True), (1000, 137, "0", 384, True),
                                                           (700, 300, "1", None, True), (900, 200, "1", None, False),
                                                           (640, 96, "0", 128, False)])
-def test_int8_gram_products_match_oracle_and_dgemm_path(monkeypatch, m, N, chunked, rows, generalized):
+def test_int8_gram_products_match_oracle_and_dgemm_path(monkeypatch, m, N, chunked, rows, generalized, bn):
     """H_a = Y^T A Y and H_b = Y^T B Y (lower triangles) through transposed digit planes and K-split INT32 accumulators
     flushed into FP64: same Ritz values / vectors / residuals as the oracle at the tolerances of
     test_rayleigh_ritz_matches_oracle, full-block and column-slab variants, several row chunks, B = I included."""
@@ -136,7 +141,7 @@ def test_int8_gram_products_match_oracle_and_dgemm_path(monkeypatch, m, N, chunk
     ritz_o, X_o, AX, BX = orc.rayleigh_ritz(A.apply, B.apply, Y)
     res_o = orc.residual_norms(AX, BX, ritz_o)
     pre = chunked == "1"
-    ritz, X, G, res, n1 = _rr(prob, Y, monkeypatch, "1", chunked, rows, gram="1", prefilter=pre)
+    ritz, X, G, res, n1 = _rr(prob, Y, monkeypatch, "1", chunked, rows, gram="1", prefilter=pre, bn=bn)
     ritz_d, X_d, G_d, res_d, n0 = _rr(prob, Y, monkeypatch, "0", chunked, rows, gram="0", prefilter=pre)
     assert n1 != n0                                                    # the INT8 kernels really ran
     Bd = prob["B"] if prob.get("B") is not None else np.eye(m)
