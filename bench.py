@@ -527,6 +527,8 @@ def main():
     ap.add_argument("--solve-method", default="rchfsi", choices=["rchfsi", "chfsi"],
                     help="method of the extra solve (chfsi = Algorithm 2 with the same kernels, the paper's comparator)")
     ap.add_argument("--solve-iters", type=int, default=60)
+    ap.add_argument("--profile-run", action="store_true",
+                    help="exit 0 even when a deliberately truncated solve (--solve-iters) is not certified: for ncu passes")
     ap.add_argument("--fe-cells", type=int, default=None, help="c4/c5: cells per direction (profiling a smaller mesh)")
     ap.add_argument("--block", type=int, default=None, help="override the block width N (profiling)")
     args = ap.parse_args()
@@ -584,7 +586,8 @@ def main():
         dist.destroy_process_group()
     if rank == 0 and isinstance(out.get("solve"), dict) and out["solve"].get("certified") is False:
         sys.stderr.write("bench.py: the configs[4] solve is NOT certified by the oracle: %s\n" % json.dumps(out["solve"]))
-        sys.exit(3)
+        if not args.profile_run:
+            sys.exit(3)
 
 
 if __name__ == "__main__":

@@ -83,6 +83,7 @@ static Knobs read_knobs() {
   k.rr_chunked = geti("RCHFSI_RR_CHUNKED", -1);
   k.rr_fe_simt = getenv("RCHFSI_RR_FE_SIMT") != nullptr;
   k.rr_timing = getenv("RCHFSI_RR_TIMING") != nullptr;
+  k.rr_fe_batched = getenv("RCHFSI_RR_FE_BATCHED") != nullptr;
   k.rr_split = geti("RCHFSI_RR_SPLIT", -1);
   k.rr_i8_rows = geti("RCHFSI_RR_I8_ROWS", 0);
   k.rr_gram_i8 = geti("RCHFSI_RR_GRAM_I8", -1);

@@ -57,6 +57,7 @@ struct Knobs {
   int dense_mc = -1;             // RCHFSI_DENSE_MC: operator-tile multicast on / off, -1 = automatic
   int rr_chunked = -1;           // RCHFSI_RR_CHUNKED: force the memory-light Rayleigh-Ritz on / off
   bool rr_fe_simt = false;       // RCHFSI_RR_FE_SIMT: FE applies of the Rayleigh-Ritz through the hand-written FP64 kernel
+  bool rr_fe_batched = false;    // RCHFSI_RR_FE_BATCHED: shared cell matrix through the batched GEMM as well (A/B knob)
   bool rr_timing = false;        // RCHFSI_RR_TIMING: print phase times of the Rayleigh-Ritz to stderr
   int rr_split = -1;             // RCHFSI_RR_SPLIT: rotation X = Y E on the INT8 tensor pipe (rr_i8.cu): 0 off, 1 forced, -1 = automatic
   int rr_gram_i8 = -1;           // RCHFSI_RR_GRAM_I8: Gram products Y^T (Op Y) on the INT8 tensor pipe: 0 off, 1 forced, -1 = automatic

@@ -16,17 +16,19 @@ namespace {
 
 // One warp per gathered row, lanes along the contiguous columns (16-byte accesses when VEC = 2).
 // Wg[bi][b][j] = W[conn[cell(bi)][b]][j]
+// (cell stride cs, node stride bs) = (n_loc N, N): one [n_loc][N] block per cell (batched GEMM), or (N, batch N): all
+// cells side by side, [n_loc][batch][N] (ONE GEMM when every cell has the same matrix)
 template <int VEC>
 __global__ void feg_gather_kernel(const double *__restrict__ W, int64_t ldw, const int32_t *__restrict__ conn,
                                   const int32_t *__restrict__ cells, int32_t n_loc, int32_t N, double *__restrict__ Wg,
-                                  int32_t rows) {
+                                  int32_t rows, int64_t cs, int64_t bs) {
   const int lane = threadIdx.x & 31;
   const int wpb = blockDim.x >> 5;
   for (int32_t r = blockIdx.x * wpb + (threadIdx.x >> 5); r < rows; r += gridDim.x * wpb) {
     const int32_t bi = r / n_loc;
     const int32_t b = r - bi * n_loc;
     const double *src = W + (int64_t)conn[(int64_t)cells[bi] * n_loc + b] * ldw;
-    double *dst = Wg + (int64_t)r * N;
+    double *dst = Wg + bi * cs + b * bs;
     if constexpr (VEC == 2) {
       for (int j = lane; j < N / 2; j += 32) reinterpret_cast<double2 *>(dst)[j] = reinterpret_cast<const double2 *>(src)[j];
     } else {
@@ -39,7 +41,7 @@ __global__ void feg_gather_kernel(const double *__restrict__ W, int64_t ldw, con
 template <int VEC>
 __global__ void feg_scatter_kernel(const double *__restrict__ Tc, const int32_t *__restrict__ conn,
                                    const uint8_t *__restrict__ flags, const int32_t *__restrict__ cells, int32_t n_loc,
-                                   int32_t N, double *__restrict__ T, int64_t ldt, int32_t rows) {
+                                   int32_t N, double *__restrict__ T, int64_t ldt, int32_t rows, int64_t cs, int64_t bs) {
   const int lane = threadIdx.x & 31;
   const int wpb = blockDim.x >> 5;
   for (int32_t r = blockIdx.x * wpb + (threadIdx.x >> 5); r < rows; r += gridDim.x * wpb) {
@@ -47,7 +49,7 @@ __global__ void feg_scatter_kernel(const double *__restrict__ Tc, const int32_t 
     const int32_t a = r - bi * n_loc;
     const int64_t e = (int64_t)cells[bi] * n_loc + a;
     double *o = T + (int64_t)conn[e] * ldt;
-    const double *src = Tc + (int64_t)r * N;
+    const double *src = Tc + bi * cs + a * bs;
     const bool first = flags[e] & 1;
     if constexpr (VEC == 2) {
       for (int j = lane; j < N / 2; j += 32) {
@@ -147,32 +149,46 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   const double one = 1.0, zero = 0.0;
   cudaStream_t st = h->stream;
   const unsigned ew = 148 * 16;
+  // (Measured and removed: gather of batch k+1 and scatter of batch k-1 on side streams under the GEMM of batch k, two
+  // half-size scratch sets -- bit-identical results, no gain: every one of the three kernels fills the GPU by itself,
+  // so they serialise anyway.  configs[3]: A Y 55.1 against 56.4 ms.)
   for (int k = 0; k < col.n_colors; ++k)
     for (int64_t b0 = col.color_begin[k]; b0 < col.color_begin[k + 1]; b0 += cap) {
       const int64_t batch = std::min<int64_t>(cap, col.color_begin[k + 1] - b0);
       const int32_t *cells = col.cell_order + b0;
       const int32_t rows = (int32_t)(batch * nl);
-      if (vec2) feg_gather_kernel<2><<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows);
-      else feg_gather_kernel<1><<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows);
+      // one matrix for every cell (a mass matrix on a uniform mesh): the cells go side by side and the colour is ONE
+      // dgemm with M = batch N instead of `batch` small ones
+      const bool one_gemm = op.cell_shared && !h->knobs.rr_fe_batched && batch * (int64_t)N < ((int64_t)1 << 31);
+      const int64_t cs = one_gemm ? N : (int64_t)nl * N, bs = one_gemm ? batch * (int64_t)N : N;
+      if (vec2) feg_gather_kernel<2><<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows, cs, bs);
+      else feg_gather_kernel<1><<<ew, 256, 0, st>>>(W, ldw, op.conn, cells, nl, N, h->feg_W, rows, cs, bs);
       LAUNCH_CHECK(h);
-      if (conv) {
+      if (conv && (!op.cell_shared || (k == 0 && b0 == col.color_begin[0]))) {
         feg_convert_kernel<<<ew, 256, 0, st>>>(op.cell_mats_f32, cells, (int64_t)nl * nl, h->feg_A, op.cell_shared ? 1 : batch, op.cell_shared ? 1 : 0);
         LAUNCH_CHECK(h);
       }
-      feg_pointers_kernel<<<(unsigned)cdiv(batch, 128), 128, 0, st>>>(h->feg_ptrs, batch, pcap, h->feg_W, h->feg_T, (int64_t)nl * N,
-                                                                      op.cell_mats, mper, cells, conv ? h->feg_A : nullptr);
-      LAUNCH_CHECK(h);
+      if (!one_gemm) {
+        feg_pointers_kernel<<<(unsigned)cdiv(batch, 128), 128, 0, st>>>(h->feg_ptrs, batch, pcap, h->feg_W, h->feg_T, (int64_t)nl * N,
+                                                                        op.cell_mats, mper, cells, conv ? h->feg_A : nullptr);
+        LAUNCH_CHECK(h);
+      }
       // row-major [nl][N] blocks are column-major N x nl: Tc (N x nl) = Wg (N x nl) * Acm (nl x nl), where the
       // column-major read of the row-major cell matrix is Acm(b, a) = A_c[a][b], so Tc[a][j] = sum_b A_c[a][b] Wg[b][j]
-      cublasStatus_t cs = cublasDgemmBatched(h->cublas, CUBLAS_OP_N, CUBLAS_OP_N, N, nl, nl, &one, h->feg_ptrs, N,
-                                             h->feg_ptrs + pcap, nl, &zero, (double **)(h->feg_ptrs + 2 * pcap), N, (int)batch);
-      if (cs != CUBLAS_STATUS_SUCCESS) {
-        h->err = "cublasDgemmBatched (FE apply): status " + std::to_string((int)cs);
+      cublasStatus_t cst;
+      if (one_gemm)
+        cst = cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_N, (int)(batch * N), nl, nl, &one, h->feg_W, (int)(batch * N),
+                          conv ? h->feg_A : op.cell_mats, nl, &zero, h->feg_T, (int)(batch * N));
+      else
+        cst = cublasDgemmBatched(h->cublas, CUBLAS_OP_N, CUBLAS_OP_N, N, nl, nl, &one, h->feg_ptrs, N, h->feg_ptrs + pcap, nl,
+                                 &zero, (double **)(h->feg_ptrs + 2 * pcap), N, (int)batch);
+      if (cst != CUBLAS_STATUS_SUCCESS) {
+        h->err = "cublasDgemm(Batched) (FE apply): status " + std::to_string((int)cst);
         return RCHFSI_ECUDA;
       }
       h->launches++;
-      if (vec2) feg_scatter_kernel<2><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows);
-      else feg_scatter_kernel<1><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows);
+      if (vec2) feg_scatter_kernel<2><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows, cs, bs);
+      else feg_scatter_kernel<1><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows, cs, bs);
       LAUNCH_CHECK(h);
     }
   return RCHFSI_OK;
