@@ -297,7 +297,8 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   }
   // Gram matrices, one column chunk of A Y / B Y at a time:  H[:, c0:c0+w] = Y^T (Op Y[:, c0:c0+w]).
   // INT8 tensor pipe (rr_i8.cu) when the filter's blocks -- dead between two filters -- can hold the transposed digit
-  // planes of Y; cuBLAS dgemm otherwise (e.g. the Rayleigh-Ritz on the initial guess, before any filter ran).
+  // planes of Y (rchfsi_solve allocates them before its first Rayleigh-Ritz); cuBLAS dgemm otherwise (a stand-alone
+  // rchfsi_rayleigh_ritz on a handle that has never filtered).
   bool g8 = false;
   if (gram_i8_supported(h) && !h->run.active) {
     std::vector<I8Buf> bufs;

@@ -78,6 +78,7 @@ def test_null_handle_is_einval_everywhere():
     assert lib.rchfsi_workspace_shortfall(None) == 0 and lib.rchfsi_workspace_used(None) == 0
     assert lib.rchfsi_operator_changed(None) == P.EINVAL
     assert lib.rchfsi_estimate_bounds(None, 10, 0, 0, None) == P.EINVAL
+    assert lib.rchfsi_rotate(None, None, None) == P.EINVAL
 
 
 def test_no_cpu_fallback_without_a_device():
@@ -111,3 +112,21 @@ def test_workspace_bytes_scales_with_the_block():
     opt.apply_prec, opt.store_prec, opt.g_input_f32 = P.BF16, P.FP32, 1
     w5 = lib.rchfsi_workspace_bytes(C.byref(fe), None, 2400, C.byref(opt), P.USE_FILTER, 50)
     assert 75e9 < w5 < (180e9 - 58.6e9 - 29.3e9)
+
+
+def test_allocation_free_entry_point_validates_before_touching_the_device():
+    """rchfsi_residual_static (static device scratch, N <= RCHFSI_STATIC_MAX_N): bad sizes and null pointers are
+    RCHFSI_EINVAL with a message that names the limit, decided on the host before any CUDA call."""
+    lib = P.load_library()
+    buf = (C.c_double * 8)()
+    p = C.cast(buf, C.c_void_p)
+    assert lib.rchfsi_residual_static(None, p, p, 4, 2, p, p, None) == P.EINVAL
+    assert b"null input" in lib.rchfsi_static_last_error()
+    assert lib.rchfsi_residual_static(p, p, p, 4, 2, None, None, None) == P.EINVAL
+    assert lib.rchfsi_residual_static(p, p, p, 0, 2, p, p, None) == P.EINVAL
+    assert lib.rchfsi_residual_static(p, p, p, 4, P.STATIC_MAX_N + 1, p, p, None) == P.EINVAL
+    msg = lib.rchfsi_static_last_error()
+    assert b"RCHFSI_STATIC_MAX_N" in msg and str(P.STATIC_MAX_N + 1).encode() in msg
+    hdr = open(os.path.join(ROOT, "include", "rchfsi.h")).read()
+    assert "#define RCHFSI_STATIC_MAX_N %d" % P.STATIC_MAX_N in hdr
+    assert "#define RCHFSI_STATIC_SCRATCH_BYTES %d" % (32 * 8 + 148 * P.STATIC_MAX_N * 8) in hdr
