@@ -11,7 +11,8 @@ operator+recurrence launches, the final combination) on one synthetic block.  Me
 Default workload: BASELINE.json configs[4], the largest single-GPU configuration (FE 24^3 cells, degree 6,
 m = 3,048,625, N = 2400, p = 50, BF16 cell-GEMM operands, FP32 recurrence blocks, FP64 X / Rayleigh-Ritz).
 The same line carries
-  "also"   one sub-record per remaining kernel claim (c2 dense TF32, c3 CSR FP32, c4 FE TF32, c4 FE BF16),
+  "also"   one sub-record per remaining kernel claim (c2 dense TF32, c3 CSR FP32, c4 FE TF32, c4 FE BF16, and the
+           Rayleigh-Ritz rotation on the INT8 tensor pipe against cuBLAS dgemm),
   "solve"  the full configs[4] R-ChFSI solve to 1e-8, certified by the ORACLE's operator on sampled columns,
   "e2e"    the same filter through rchfsi_filter_host (pinned host buffers, column-chunked pipeline),
   "cpu_baseline"  the oracle's filter on a bounded sample on the host cores.
@@ -333,6 +334,67 @@ def time_e2e(solver, P, Xh, rh, Gh, p, bounds, reps, dev, world):
     return float(te.item()), int(h2d), int(Xh.numel() * 8)
 
 
+def bench_rotation(dev, m=262144, N=2400, reps=5):
+    """Sub-record for the Rayleigh-Ritz rotation X = Y E: rchfsi_rotate on a seeded block, INT8
+    tensor-pipe path (default) and cuBLAS dgemm (RCHFSI_RR_SPLIT=0) on the same inputs; FP64-equivalent flops = 2 m N^2.
+    The INT8 path does 28 digit-plane products per FP64 product: achieved INT8 rate = 28 x 2 m N^2 ops / time."""
+    import torch
+    import paper_2503_22652_b200 as P
+    g = torch.Generator(device=dev).manual_seed(11)
+    Y0 = torch.randn((m, N), dtype=torch.float64, device=dev, generator=g)
+    E = torch.linalg.qr(torch.randn((N, N), dtype=torch.float64, device=dev, generator=g))[0].contiguous()
+    ident = dict(kind="csr", rowptr=torch.arange(m + 1, dtype=torch.int64, device=dev),
+                 colind=torch.arange(m, dtype=torch.int32, device=dev), vals=torch.ones(m, dtype=torch.float64, device=dev))
+    times, outs = {}, {}
+    for name, knob in (("int8", None), ("dgemm", "0")):
+        old = os.environ.get("RCHFSI_RR_SPLIT")
+        if knob is None:
+            os.environ.pop("RCHFSI_RR_SPLIT", None)
+        else:
+            os.environ["RCHFSI_RR_SPLIT"] = knob
+        try:
+            s = P.Rchfsi(ident, None, None, block_N=N)       # knobs are read when the handle is created
+        finally:
+            if old is None:
+                os.environ.pop("RCHFSI_RR_SPLIT", None)
+            else:
+                os.environ["RCHFSI_RR_SPLIT"] = old
+        Y = Y0.clone()
+        s.rotate(Y, E)
+        outs[name] = Y[:512].clone()
+        best = None
+        sampler = ClockSampler(torch.cuda.current_device())
+        sampler.start()
+        for _ in range(reps):
+            Y.copy_(Y0)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            s.rotate(Y, E)
+            e1.record()
+            torch.cuda.synchronize()
+            t = e0.elapsed_time(e1)
+            best = t if best is None else min(best, t)
+        clocks = sampler.finish()
+        times[name] = (best, clocks)
+        s.close()
+        del Y
+    peaks = load_peaks()
+    bf16 = peaks.get("bf16_tflops", 1590.0)
+    flops = 2.0 * m * N * N
+    ms = times["int8"][0]
+    dev_max = float((outs["int8"] - outs["dgemm"]).abs().max() / outs["dgemm"].abs().max())
+    return {"metric": "Rayleigh-Ritz rotation X = Y E, FP64-equivalent TFLOP/s", "value": flops / (ms * 1e-3) / 1e12, "unit": "TFLOP/s",
+            "ms": ms, "dgemm_ms": times["dgemm"][0], "dgemm_value": flops / (times["dgemm"][0] * 1e-3) / 1e12,
+            "speedup_vs_dgemm": times["dgemm"][0] / ms, "max_rel_dev_vs_dgemm": dev_max, "dtype": "int8 digits -> f64",
+            "config": {"workload": "rotation of a seeded %d x %d block by a %d x %d orthogonal matrix" % (m, N, N, N)},
+            "clocks": times["int8"][1],
+            "roofline": {"bound": "tensor", "achieved": 28.0 * flops / (ms * 1e-3) / 1e12, "peak": 2.0 * bf16, "unit": "TOP/s",
+                         "frac": 28.0 * flops / (ms * 1e-3) / 1e12 / (2.0 * bf16),
+                         "kernel": "i8w_kernel<0> (tcgen05.mma kind::i8, 28 digit-plane products per FP64 product)",
+                         "peak_source": "MEASURED_PEAKS.json bf16 burst x 2 (nominal INT8/BF16 ratio)", "traffic": None}}
+
+
 def bench_resident(key, apply_prec, store_prec, steps, warmup, dev, rank, world, want_e2e, want_cpu, want_solve, args):
     """configs[0..3]: inputs of Alg. 3 (B-orthonormal X, Ritz values, G) from one rchfsi_rayleigh_ritz on the seeded
     start block; filter timed with the inputs resident in HBM, L2 flushed between timed calls."""
@@ -578,6 +640,11 @@ def main():
             except Exception as exc:     # one failing sub-record must not lose the line
                 also[key] = {"error": "%s: %s" % (type(exc).__name__, exc)}
                 torch.cuda.empty_cache()
+        try:
+            also["rr_rotation_int8"] = bench_rotation(dev)
+        except Exception as exc:
+            also["rr_rotation_int8"] = {"error": "%s: %s" % (type(exc).__name__, exc)}
+        torch.cuda.empty_cache()
         out["also"] = also
     out["wall_s_total"] = time.perf_counter() - t_start
     if rank == 0:

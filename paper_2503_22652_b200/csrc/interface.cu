@@ -29,11 +29,6 @@ __device__ __forceinline__ void st_prec(void *p, int64_t i, int prec, double v) 
   if (prec == RCHFSI_FP64) reinterpret_cast<double *>(p)[i] = v;
   else reinterpret_cast<float *>(p)[i] = (float)v;
 }
-__device__ __forceinline__ double wire_round(double v, int wire) {
-  if (wire == RCHFSI_BF16) return (double)__bfloat162float(__float2bfloat16_rn((float)v));
-  if (wire == RCHFSI_FP32) return (double)(float)v;
-  return v;
-}
 __device__ __forceinline__ void st_wire(void *p, int64_t i, int wire, double v) {
   if (wire == RCHFSI_BF16) reinterpret_cast<__nv_bfloat16 *>(p)[i] = __float2bfloat16_rn((float)v);
   else if (wire == RCHFSI_FP32) reinterpret_cast<float *>(p)[i] = (float)v;

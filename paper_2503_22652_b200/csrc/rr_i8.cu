@@ -489,6 +489,7 @@ struct I8WParams {
   int32_t zc0;             // tiles with a0 + 127 < zc0 + (packed ? 0 : b0) are skipped
   int32_t packed;          // N side = several column slabs side by side (all at global column zc0)
   int32_t accumulate;      // the first drain adds to Hpart as well (row chunks after the first)
+  int32_t debug_mode;      // -DRCHFSI_PROBES builds: 1 = no TMA loads (MMA rate), 2 = no MMAs (operand-stream rate)
 };
 
 // one drain of the accumulators of a pass into the thread's FP64 registers: NACC = 4 (anti-diagonals 0..3) or 3 (4..6,
@@ -576,8 +577,12 @@ __global__ void __launch_bounds__(320, 1) i8w_kernel(const __grid_constant__ I8M
               const int slot = ib % I8W_SLOTS;
               mbar_wait(b_empty + slot, ((ib / I8W_SLOTS) & 1) ^ 1);
               if (elect_one()) {
-                mbar_expect_tx(b_full + slot, I8W_TILE);
-                tma_load_2d(Bs + slot * I8W_TILE, &mapsB.m[t], b_full + slot, k0, b0);
+                if (PROBE(p.debug_mode, 1)) {
+                  mbar_arrive(b_full + slot);
+                } else {
+                  mbar_expect_tx(b_full + slot, I8W_TILE);
+                  tma_load_2d(Bs + slot * I8W_TILE, &mapsB.m[t], b_full + slot, k0, b0);
+                }
               }
               __syncwarp();
             }
@@ -585,8 +590,12 @@ __global__ void __launch_bounds__(320, 1) i8w_kernel(const __grid_constant__ I8M
             const int slot = ia % I8W_SLOTS;
             mbar_wait(a_empty + slot, ((ia / I8W_SLOTS) & 1) ^ 1);
             if (elect_one()) {
-              mbar_expect_tx(a_full + slot, I8W_TILE);
-              tma_load_2d(As + slot * I8W_TILE, &mapsA.m[s], a_full + slot, k0, a0);
+              if (PROBE(p.debug_mode, 1)) {
+                mbar_arrive(a_full + slot);
+              } else {
+                mbar_expect_tx(a_full + slot, I8W_TILE);
+                tma_load_2d(As + slot * I8W_TILE, &mapsA.m[s], a_full + slot, k0, a0);
+              }
             }
             __syncwarp();
           }
@@ -622,6 +631,7 @@ __global__ void __launch_bounds__(320, 1) i8w_kernel(const __grid_constant__ I8M
               const uint64_t da = da0 + (uint32_t)(((ia % I8W_SLOTS) * I8W_TILE) >> 4);
               const int t_hi = dhi - s, t_lo = dlo - s > 0 ? dlo - s : 0;
               for (int t = t_hi; t >= t_lo; --t) {
+                if (PROBE(p.debug_mode, 2)) break;
                 const int ib = it + (dhi - t);
                 const uint64_t db = db0 + (uint32_t)(((ib % I8W_SLOTS) * I8W_TILE) >> 4);
 #pragma unroll
@@ -765,6 +775,7 @@ rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const dou
       I8WParams p{};
       p.MA = (int32_t)rc; p.NB = N; p.num_k_blocks = (int32_t)cdiv(N, 128);
       p.Out = Out + (size_t)r0 * N; p.ldo = N; p.ea = ea; p.eb = eb;
+      p.debug_mode = h->knobs.tc_debug;
       dim3 grid((unsigned)cdiv(N, I8W_BN), (unsigned)cdiv(rc, 128), 1);
       i8w_kernel<0><<<grid, 320, I8W_SMEM, st>>>(ma, mb, p);
       LAUNCH_CHECK(h);
@@ -872,6 +883,7 @@ rchfsi_status gram_launch(rchfsi_ctx *h, const I8Planes &yp, const I8Planes &zp,
     I8WParams p{};
     p.MA = h->N; p.NB = Nz; p.num_k_blocks = (int32_t)cdiv(rows, 128);
     p.Hpart = reinterpret_cast<double *>(h->i8_hpart); p.zc0 = zc0; p.packed = packed ? 1 : 0; p.accumulate = accumulate ? 1 : 0;
+    p.debug_mode = h->knobs.tc_debug;
     dim3 grid((unsigned)cdiv(Nz, I8W_BN), (unsigned)cdiv(h->N, 128), (unsigned)KS);
     i8w_kernel<1><<<grid, 320, I8W_SMEM, h->stream>>>(ma, mb, p);
     LAUNCH_CHECK(h);
