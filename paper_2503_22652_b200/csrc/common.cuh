@@ -162,6 +162,7 @@ struct rchfsi_ctx {
   float *Gsolve32 = nullptr;                               // [m][N] FP32 residual block of rchfsi_solve (chunked mode)
   double *feg_W = nullptr, *feg_T = nullptr, *feg_A = nullptr;  // fe_rr.cu scratch: gathered operand, product, FP64 cell batch
   const double **feg_ptrs = nullptr;                        // [3][feg_ptr_cap] pointer arrays of the batched GEMM
+  const double *feg_A_full = nullptr;                       // FP64 copy of all FP32 cell matrices, lent for one Rayleigh-Ritz
   size_t feg_w_bytes = 0, feg_W_bytes = 0, feg_T_bytes = 0; int64_t feg_a_cells = 0, feg_ptr_cap = 0; int32_t feg_N = 0;
   double *Ha = nullptr, *Hb = nullptr;                     // [N][N]
   void *i8_cols = nullptr, *i8_hpart = nullptr; size_t i8_hpart_bytes = 0;   // rr_i8.cu: column maxima / exponents, K-split partial Gram sums
@@ -329,6 +330,8 @@ bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op);
 // T = Op W in FP64 through gather -> batched DGEMM -> coloured scatter (Rayleigh-Ritz only)
 rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,
                             int64_t ldw = 0, int64_t ldt = 0);
+size_t fe_rr_fp64_cells_bytes(const rchfsi_ctx *h);            // 0 unless A is an FP32-only FE operator
+rchfsi_status fe_rr_lend_fp64_cells(rchfsi_ctx *h, void *buf); // valid until the caller resets h->feg_A_full
 
 // ---- rr.cu -----------------------------------------------------------------------------
 rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, double *G_out,
@@ -351,7 +354,8 @@ bool gram_i8_supported(const rchfsi_ctx *h);
 size_t rr_i8_plan_bytes(int64_t m, int32_t N);   // digit planes of E, column exponents, K-split partial sums
 rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, const double *BY, double *Ha, double *Hb,
                            void *scratch, size_t scratch_bytes);
-bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int32_t max_w, rchfsi_status *st);
+bool carve_buf(std::vector<I8Buf> &bufs, size_t bytes, void **out);   // first fit, 256-byte aligned; consumes what it returns
+bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> &bufs, int32_t max_w, rchfsi_status *st);
 rchfsi_status gram_i8_slab(rchfsi_ctx *h, const double *Y, const double *Z1, const double *Z2, int64_t ldz, int32_t w, int32_t zc0,
                            double *Ha, double *Hb);
 

@@ -72,7 +72,7 @@ __global__ void feg_convert_kernel(const float *__restrict__ mats, const int32_t
   const int64_t total = batch * per;
   for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
     const int64_t bi = t / per;
-    out[t] = (double)mats[(shared ? 0 : (int64_t)cells[bi]) * per + (t - bi * per)];
+    out[t] = (double)mats[(shared ? 0 : (cells ? (int64_t)cells[bi] : bi)) * per + (t - bi * per)];
   }
 }
 
@@ -118,7 +118,11 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
   RCHFSI_TRY(fe_ensure_coloring(h));
   const FeColoring &col = h->coloring;
   const int32_t nl = op.n_loc;
-  const bool conv = (op.cell_mats == nullptr);
+  // FP64 cell matrices: the caller's, or (FP32-only operators) the copy the Rayleigh-Ritz parked in the filter's dead
+  // blocks for the duration of one call (fe_rr_lend_fp64_cells), or else a per-batch conversion
+  const double *mats64 = op.cell_mats;
+  if (!mats64 && h->feg_A_full && &op == &h->A.d) mats64 = h->feg_A_full;
+  const bool conv = (mats64 == nullptr);
   const int64_t mper = op.cell_shared ? 0 : (int64_t)nl * nl;
   // scratch: gathered operand + product (+ FP64 copy of FP32 cell matrices), about 1.5 GB; sized once for the widest
   // block the handle can see (N_cap or the chunk width of the memory-light Rayleigh-Ritz)
@@ -170,7 +174,7 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
       }
       if (!one_gemm) {
         feg_pointers_kernel<<<(unsigned)cdiv(batch, 128), 128, 0, st>>>(h->feg_ptrs, batch, pcap, h->feg_W, h->feg_T, (int64_t)nl * N,
-                                                                        op.cell_mats, mper, cells, conv ? h->feg_A : nullptr);
+                                                                        mats64, mper, cells, conv ? h->feg_A : nullptr);
         LAUNCH_CHECK(h);
       }
       // row-major [nl][N] blocks are column-major N x nl: Tc (N x nl) = Wg (N x nl) * Acm (nl x nl), where the
@@ -178,7 +182,7 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
       cublasStatus_t cst;
       if (one_gemm)
         cst = cublasDgemm(h->cublas, CUBLAS_OP_N, CUBLAS_OP_N, (int)(batch * N), nl, nl, &one, h->feg_W, (int)(batch * N),
-                          conv ? h->feg_A : op.cell_mats, nl, &zero, h->feg_T, (int)(batch * N));
+                          conv ? h->feg_A : mats64, nl, &zero, h->feg_T, (int)(batch * N));
       else
         cst = cublasDgemmBatched(h->cublas, CUBLAS_OP_N, CUBLAS_OP_N, N, nl, nl, &one, h->feg_ptrs, N, h->feg_ptrs + pcap, nl,
                                  &zero, (double **)(h->feg_ptrs + 2 * pcap), N, (int)batch);
@@ -191,6 +195,22 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
       else feg_scatter_kernel<1><<<ew, 256, 0, st>>>(h->feg_T, op.conn, col.flags, cells, nl, N, T, ldt, rows, cs, bs);
       LAUNCH_CHECK(h);
     }
+  return RCHFSI_OK;
+}
+
+// FP64 copy of ALL cell matrices of an FP32-only operator A into `buf` (n_cells n_loc^2 doubles, lent by the caller for
+// the duration of one Rayleigh-Ritz): every operator apply of that call then skips its per-batch conversion.
+size_t fe_rr_fp64_cells_bytes(const rchfsi_ctx *h) {
+  const rchfsi_operator &A = h->A.d;
+  if (A.kind != RCHFSI_OP_FE || A.cell_mats || !A.cell_mats_f32 || A.cell_shared) return 0;
+  return sizeof(double) * (size_t)A.n_cells * A.n_loc * A.n_loc;
+}
+rchfsi_status fe_rr_lend_fp64_cells(rchfsi_ctx *h, void *buf) {
+  const rchfsi_operator &A = h->A.d;
+  feg_convert_kernel<<<148 * 16, 256, 0, h->stream>>>(A.cell_mats_f32, nullptr, (int64_t)A.n_loc * A.n_loc,
+                                                     reinterpret_cast<double *>(buf), A.n_cells, 0);
+  LAUNCH_CHECK(h);
+  h->feg_A_full = reinterpret_cast<const double *>(buf);
   return RCHFSI_OK;
 }
 

@@ -299,15 +299,27 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   // INT8 tensor pipe (rr_i8.cu) when the filter's blocks -- dead between two filters -- can hold the transposed digit
   // planes of Y (rchfsi_solve allocates them before its first Rayleigh-Ritz); cuBLAS dgemm otherwise (a stand-alone
   // rchfsi_rayleigh_ritz on a handle that has never filtered).
-  bool g8 = false;
-  if (gram_i8_supported(h) && !h->run.active) {
-    std::vector<I8Buf> bufs;
+  // The filter's blocks R_X, R_Y and the operand shadow are dead between two filters (the filter re-initialises them):
+  // this call borrows them for the transposed digit planes and for an FP64 copy of FP32-only cell matrices.
+  struct Borrowed {
+    rchfsi_ctx *h;
+    ~Borrowed() { h->i8g.active = false; h->feg_A_full = nullptr; }
+  } borrowed{h};
+  std::vector<I8Buf> bufs;
+  if (!h->run.active) {
     if (h->RX) bufs.push_back({h->RX, h->RX_bytes});
     if (h->RY) bufs.push_back({h->RY, h->RY_bytes});
     if (h->Wa) bufs.push_back({h->Wa, h->Wa_bytes});
+  }
+  bool g8 = false;
+  if (gram_i8_supported(h) && !bufs.empty()) {
     rchfsi_status gst = RCHFSI_OK;
     g8 = gram_i8_begin(h, Y, bufs, cw, &gst);
     if (gst != RCHFSI_OK) return gst;
+  }
+  if (const size_t cb = fe_rr_fp64_cells_bytes(h)) {     // converted once per call instead of once per batch and chunk
+    void *cells64 = nullptr;
+    if (carve_buf(bufs, cb, &cells64)) RCHFSI_TRY(fe_rr_lend_fp64_cells(h, cells64));
   }
   for (int32_t c0 = 0; c0 < N; c0 += cw) {
     const int32_t w = std::min(cw, N - c0);
@@ -326,7 +338,6 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
                                 h->Hb + (size_t)c0 * N + c0, N));
     h->launches += 2;
   }
-  h->i8g.active = false;
   pt.lap("chunked: applies + Gram (lower)");
   CUSOLVER_CHECK(h, cusolverDnDsygvd(h->cusolver, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
                                      CUBLAS_FILL_MODE_LOWER, N, h->Ha, N, h->Hb, N, h->ritz_dev, h->sy_work,

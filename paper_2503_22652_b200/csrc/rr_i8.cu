@@ -812,9 +812,7 @@ bool gram_i8_supported(const rchfsi_ctx *h) {
   return h->N >= 256 && h->m >= 8192;
 }
 
-namespace {
-
-bool carve(std::vector<I8Buf> &bufs, size_t bytes, void **out) {
+bool carve_buf(std::vector<I8Buf> &bufs, size_t bytes, void **out) {
   for (I8Buf &b : bufs) {
     const size_t off = (256 - (reinterpret_cast<uintptr_t>(b.ptr) & 255)) & 255;
     if (b.bytes >= bytes + off) {
@@ -826,6 +824,8 @@ bool carve(std::vector<I8Buf> &bufs, size_t bytes, void **out) {
   }
   return false;
 }
+
+namespace {
 
 // column maxima (bit patterns) and exponents: Y [N], Z [2 N] (two slabs side by side)
 rchfsi_status i8_fixed(rchfsi_ctx *h) {
@@ -969,17 +969,19 @@ rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, con
 // caller's buffers (the filter's dead blocks), then every column slab contributes H_a[:, c0:c0+w] = Y^T (A Y_c) and
 // H_b[:, c0:c0+w] = Y^T (B Y_c) in ONE launch (the two slabs side by side on the N side: Y's planes are read once).
 // Returns false (nothing launched) when the buffers cannot hold the planes.
-bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> bufs, int32_t max_w, rchfsi_status *st) {
+bool gram_i8_begin(rchfsi_ctx *h, const double *Y, std::vector<I8Buf> &bufs, int32_t max_w, rchfsi_status *st) {
   *st = RCHFSI_OK;
   const int32_t N = h->N;
   const int64_t m = h->m;
   const int64_t Rp = (m + 127) / 128 * 128;
   I8GramState &g = h->i8g;
   g.active = false;
+  std::vector<I8Buf> trial = bufs;
   for (int s = 0; s < I8_S; ++s)
-    if (!carve(bufs, (size_t)N * Rp, reinterpret_cast<void **>(&g.yp[s]))) return false;
+    if (!carve_buf(trial, (size_t)N * Rp, reinterpret_cast<void **>(&g.yp[s]))) return false;
   for (int s = 0; s < I8_S; ++s)
-    if (!carve(bufs, (size_t)2 * max_w * Rp, reinterpret_cast<void **>(&g.zp[s]))) return false;
+    if (!carve_buf(trial, (size_t)2 * max_w * Rp, reinterpret_cast<void **>(&g.zp[s]))) return false;
+  bufs = trial;                                           // only a successful placement consumes the caller's buffers
   g.Rp = Rp;
   g.max_w = max_w;
   if ((*st = i8_fixed(h)) != RCHFSI_OK) return false;

@@ -687,6 +687,43 @@ def test_memory_light_solve_keeps_fp32_residual_block(monkeypatch, apply_prec):
     sol.close()
 
 
+@pytest.mark.parametrize("i8", ["0", "1"])
+def test_memory_light_solve_with_fp32_only_cells_borrows_the_filter_blocks(monkeypatch, i8):
+    """configs[4] storage: FP32-only cell matrices, chunked Rayleigh-Ritz.  Inside rchfsi_solve the Rayleigh-Ritz parks
+    an FP64 copy of the cell matrices (and, with the INT8 Gram products forced at this size, the transposed digit planes
+    of Y) in the filter's blocks R_X / R_Y / shadow, which the next filter re-initialises.  Converges to the eigenvalues
+    of the FP32-rounded operator (the operator the library was given), residual <= 1e-8."""
+    torch = _torch()
+    import scipy.linalg as sla
+    import paper_2503_22652_b200 as P
+    monkeypatch.setenv("RCHFSI_RR_CHUNKED", "1")
+    monkeypatch.setenv("RCHFSI_RR_GRAM_I8", i8)
+    monkeypatch.setenv("RCHFSI_RR_SPLIT", i8)
+    # 27 cells of 64 nodes, m = 1000: the FP64 cell copy (885 KB) fits the 1 MB block R_Y of the FP64-storage filter
+    prob = dict(workloads.fe_problem(3, q=3, seed=11))
+    prob["A_cells"] = prob["A_cells"].astype(np.float32).astype(np.float64)
+    A, B, Dinv = oracle_ops(prob)
+    m = prob["m"]
+    ev = sla.eigh(A.apply(np.eye(m)), B.apply(np.eye(m)), eigvals_only=True)
+    lam_max = workloads.fe.fe_lam_max_bound(prob["A_cells"], prob["B_cell"]) * 1.01
+    N, nw, p = 16, 8, 30
+    assert prob["n_cells"] * prob["n_loc"] ** 2 * 8 <= m * 128 * 8
+    X0 = np.random.default_rng(2).standard_normal((m, N))
+    As, Bs, dinv = P.upload_problem(prob, fe_cells_f32_only=True)
+    sol = P.Rchfsi(As, Bs, dinv, block_N=N, apply_prec="tf32", store_prec="fp64", adaptive_bounds=True)
+    X = torch.as_tensor(X0).cuda()
+    out = sol.solve(P.METHOD_RCHFSI, X, nw, p, ev[0] - 1.0, ev[N], lam_max, tol=1e-8, max_iter=80)
+    assert out["converged"], out["history"][-5:]
+    np.testing.assert_allclose(out["evals"][:nw], ev[:nw], rtol=1e-8, atol=1e-9)
+    assert out["resnorm"][:nw].max() <= 1e-8
+    # certified by the oracle's operators on the returned pairs
+    Xh = X[:, :nw].cpu().numpy()
+    BX = B.apply(Xh)
+    assert np.linalg.norm(A.apply(Xh) - BX * out["evals"][:nw][None, :], axis=0).max() <= 1.01e-8
+    assert np.abs(Xh.T @ BX - np.eye(nw)).max() <= 1e-9
+    sol.close()
+
+
 @pytest.mark.parametrize("f32_cells", [False, True])
 @pytest.mark.parametrize("chunked", ["0", "1"])
 def test_fe_rayleigh_ritz_batched_gemm_apply_equals_handwritten_apply(monkeypatch, f32_cells, chunked):
