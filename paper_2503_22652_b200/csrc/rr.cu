@@ -286,7 +286,6 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   // (each buffer has its own guard: the call may be repeated after the caller added workspace)
   if (!h->rrc1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)m * h->rr_cw));
   if (!h->rrc2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc2, sizeof(double) * (size_t)m * h->rr_cw));
-  if (!h->rrp) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)h->rr_rp * N));
   const int32_t cw = h->rr_cw;
   h->feg_N = std::max(h->feg_N, cw);    // FE apply scratch sized once for the chunk width
   const double one = 1.0, zero = 0.0;
@@ -317,9 +316,28 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     g8 = gram_i8_begin(h, Y, bufs, cw, &gst);
     if (gst != RCHFSI_OK) return gst;
   }
+  const uint8_t *cells64 = nullptr;
   if (const size_t cb = fe_rr_fp64_cells_bytes(h)) {     // converted once per call instead of once per batch and chunk
-    void *cells64 = nullptr;
-    if (carve_buf(bufs, cb, &cells64)) RCHFSI_TRY(fe_rr_lend_fp64_cells(h, cells64));
+    void *pc = nullptr;
+    if (carve_buf(bufs, cb, &pc)) {
+      RCHFSI_TRY(fe_rr_lend_fp64_cells(h, pc));
+      cells64 = reinterpret_cast<const uint8_t *>(pc);
+    }
+  }
+  // scratch of the rotation (digit planes of a row chunk of Y): the largest borrowed block that does not hold the cell
+  // copy -- by then the transposed planes of the Gram products are dead; the row panel only when nothing can be borrowed
+  void *rot_buf = nullptr;
+  size_t rot_bytes = 0;
+  if (!h->run.active)
+    for (const I8Buf &b : {I8Buf{h->RX, h->RX_bytes}, I8Buf{h->RY, h->RY_bytes}, I8Buf{h->Wa, h->Wa_bytes}}) {
+      const uint8_t *p0 = reinterpret_cast<const uint8_t *>(b.ptr);
+      if (p0 && !(cells64 && cells64 >= p0 && cells64 < p0 + b.bytes) && b.bytes > rot_bytes) { rot_buf = b.ptr; rot_bytes = b.bytes; }
+    }
+  const bool rot8 = rotate_i8_supported(h);
+  if (!(rot8 && rot_buf)) {
+    if (!h->rrp) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)h->rr_rp * N));
+    rot_buf = h->rrp;
+    rot_bytes = sizeof(double) * (size_t)h->rr_rp * N;
   }
   for (int32_t c0 = 0; c0 < N; c0 += cw) {
     const int32_t w = std::min(cw, N - c0);
@@ -354,8 +372,8 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
   pt.lap("chunked: dsygvd");
   const double *E = h->Ha;
   // X = Y E in place, one row panel at a time (row-major rows r0.. are the columns r0.. of the N x m view)
-  if (rotate_i8_supported(h)) {
-    RCHFSI_TRY(rotate_i8(h, Y, m, E, Y, h->rrp, sizeof(double) * (size_t)h->rr_rp * N));   // the panel holds the digit planes
+  if (rot8) {
+    RCHFSI_TRY(rotate_i8(h, Y, m, E, Y, rot_buf, rot_bytes));
   } else {
     for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
       const int64_t rows = std::min<int64_t>(h->rr_rp, m - r0);

@@ -47,6 +47,18 @@ __host__ __device__ constexpr uint32_t make_idesc_i8(int M, int N) {
   return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
+// Balanced base-256 digits without a loop: q = sum_k d_k 256^k with d_k in [-128, 127] is the same as
+// q + sum_k 128 256^k = sum_k (d_k + 128) 256^k with plain unsigned digits, so byte k of b = q + 0x0080808080808080 is
+// d_k + 128 and d_k is that byte with its top bit flipped.  Digit k (0 = least significant) of four values at once:
+constexpr unsigned long long I8_BIAS = 0x0080808080808080ull;
+__device__ __forceinline__ uint32_t i8_digits(const uint32_t (&lo)[4], const uint32_t (&hi)[4], int k) {
+  const uint32_t *w = k < 4 ? lo : hi;
+  const uint32_t sel = 0x0040u + (uint32_t)(k & 3) * 0x0011u;          // bytes k of the first and of the second operand
+  const uint32_t p01 = __byte_perm(w[0], w[1], sel);
+  const uint32_t p23 = __byte_perm(w[2], w[3], sel);
+  return __byte_perm(p01, p23, 0x5410u) ^ 0x80808080u;
+}
+
 // One warp per row of V ([rows][K], row pitch ld): row exponent, then the 7 digit planes planes[s][row][Kp].
 // Columns K..Kp-1 of the planes are zero (Kp = K rounded up to 16: TMA row pitch).
 __global__ void __launch_bounds__(256) i8_slice_kernel(const double *__restrict__ V, int64_t ld, int64_t rows, int32_t K,
@@ -72,22 +84,18 @@ __global__ void __launch_bounds__(256) i8_slice_kernel(const double *__restrict_
   const size_t plane = (size_t)plane_rows * Kp;
   int8_t *out = planes + (size_t)row * Kp;
   for (int k4 = lane * 4; k4 < Kp; k4 += 128) {
-    uint32_t packed[I8_S];
-#pragma unroll
-    for (int s = 0; s < I8_S; ++s) packed[s] = 0u;
+    uint32_t lo[4], hi[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int k = k4 + u;
-      long long q = (k < K && !bad) ? __double2ll_rn(scalbn(v[k], 54 - e)) : 0ll;
-#pragma unroll
-      for (int s = I8_S - 1; s >= 0; --s) {     // least significant digit first
-        const int d = (int)(int8_t)(q & 0xff);
-        q = (q - d) >> 8;
-        packed[s] |= (uint32_t)(d & 0xff) << (8 * u);
-      }
+      const long long q = (k < K && !bad) ? __double2ll_rn(scalbn(v[k], 54 - e)) : 0ll;
+      const unsigned long long b = (unsigned long long)q + I8_BIAS;      // bytes of b = digits + 128 (see i8_digits)
+      lo[u] = (uint32_t)b;
+      hi[u] = (uint32_t)(b >> 32);
     }
 #pragma unroll
-    for (int s = 0; s < I8_S; ++s) *reinterpret_cast<uint32_t *>(out + s * plane + k4) = packed[s];
+    for (int s = 0; s < I8_S; ++s)
+      *reinterpret_cast<uint32_t *>(out + s * plane + k4) = i8_digits(lo, hi, I8_S - 1 - s);
   }
 }
 
@@ -265,17 +273,20 @@ __global__ void __launch_bounds__(256) i8_slice_t_kernel(const double *__restric
   const double cm = __longlong_as_double((long long)bits);
   const int e = (cm > 0.0 && !bad) ? ilogb(cm) + 1 : 0;
   if (blockIdx.y == 0 && w == 0 && cok && expo) expo[col] = bad ? I8_NAN_ROW : e;
-#pragma unroll 4
-  for (int i = 0; i < 16; ++i) {
-    const int rl = w + 8 * i;
-    const int64_t r = (int64_t)blockIdx.y * 128 + rl;
-    long long q = (cok && !bad && r < rows) ? __double2ll_rn(scalbn(V[(r0 + r) * ld + col], 54 - e)) : 0ll;
+#pragma unroll 2
+  for (int i = 0; i < 4; ++i) {
+    const int rl = 4 * (w + 8 * i);                        // this thread: rows rl .. rl+3 of its column
+    uint32_t lo[4], hi[4];
 #pragma unroll
-    for (int s = I8_S - 1; s >= 0; --s) {
-      const int d = (int)(int8_t)(q & 0xff);
-      q = (q - d) >> 8;
-      reinterpret_cast<uint8_t *>(&tile[s][lane][0])[rl] = (uint8_t)d;
+    for (int u = 0; u < 4; ++u) {
+      const int64_t r = (int64_t)blockIdx.y * 128 + rl + u;
+      const long long q = (cok && !bad && r < rows) ? __double2ll_rn(scalbn(V[(r0 + r) * ld + col], 54 - e)) : 0ll;
+      const unsigned long long b = (unsigned long long)q + I8_BIAS;
+      lo[u] = (uint32_t)b;
+      hi[u] = (uint32_t)(b >> 32);
     }
+#pragma unroll
+    for (int s = 0; s < I8_S; ++s) tile[s][lane][rl >> 2] = i8_digits(lo, hi, I8_S - 1 - s);
   }
   __syncthreads();
   const int64_t roff = (int64_t)blockIdx.y * 128 + lane * 4;
