@@ -243,9 +243,9 @@ rchfsi_status rchfsi_rayleigh_ritz(rchfsi_handle h, double *Y_in_X_out, double *
 /* The subspace rotation of the Rayleigh-Ritz step on its own ("X = Y E"): Y <- Y E in place, FP64.
  *  Y_in_X_out    device [m][N] row-major.
  *  E_colmajor    device N x N, column-major (the LAPACK / cuSOLVER eigenvector layout), not aliasing Y.
- * Same kernel choice as inside rchfsi_rayleigh_ritz: the INT8 tensor-pipe product of rr_i8.cu for large blocks
- * (error-free digit split of both operands, result within a few FP64 ulps of (row max of Y) x (column max of E) per
- * element), cuBLAS dgemm otherwise; RCHFSI_RR_SPLIT=0/1 forces the choice.  Asynchronous. */
+ * Same kernel as inside rchfsi_rayleigh_ritz: the INT8 tensor-pipe product of rr_i8.cu (error-free digit split of both
+ * operands, result within a few FP64 ulps of (row max of Y) x (column max of E) per element; N <= 16384);
+ * RCHFSI_RR_SPLIT=0 selects cuBLAS dgemm instead.  Asynchronous. */
 rchfsi_status rchfsi_rotate(rchfsi_handle h, double *Y_in_X_out, const double *E_colmajor);
 
 /* Algorithm 1, do-while reading: one Rayleigh-Ritz on the initial guess,

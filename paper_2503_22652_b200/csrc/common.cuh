@@ -345,6 +345,7 @@ rchfsi_status rotate_in_place(rchfsi_ctx *h, double *Y, const double *E);   // r
 
 // ---- rr_i8.cu: rotation X = Y E on the INT8 tensor pipe (error-free digit split of the FP64 operands) ----
 bool rotate_i8_supported(const rchfsi_ctx *h);
+bool rr_i8_scratch_ok(const rchfsi_ctx *h, size_t bytes);   // enough scratch for one 128-row chunk of digit planes
 size_t rotate_i8_fixed_bytes(int32_t N);        // digit planes of E, held by the handle
 // Out[r][:] = In[r][:] E for r < rows (E column-major N x N); Out may be In; `scratch` holds one row chunk's planes
 rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const double *E, double *Out, void *scratch,

@@ -1,7 +1,8 @@
 // Rayleigh-Ritz on a non-orthogonal basis, FP64 throughout.
-// Off the hot path: the Gram products are plain library GEMMs (cuBLAS dgemm), the rotation
-// X = Y E runs on the INT8 tensor pipe for large blocks (rr_i8.cu, dgemm otherwise), the N x N generalized
-// eigenproblem is cuSOLVER dsygvd; the operator applies are this library's FP64 kernels.
+// Off the hot path: the Gram products and the rotations run on the INT8 tensor pipe
+// (rr_i8.cu; cuBLAS dgemm behind RCHFSI_RR_SPLIT=0 / RCHFSI_RR_GRAM_I8=0 and for problems of a few hundred rows), the
+// N x N generalized eigenproblem is cuSOLVER dsygvd; the operator applies are this library's FP64 kernels (FE: gather,
+// cuBLAS batched dgemm with the exact cell matrices, coloured scatter).
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -160,7 +161,8 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
     BY = h->rr2;
   }
   pt.lap("B Y");
-  if (gram_i8_supported(h)) {   // rr3 holds the transposed digit planes until the rotation needs it
+  const bool i8ok = rr_i8_scratch_ok(h, blk);
+  if (gram_i8_supported(h) && i8ok) {   // rr3 holds the transposed digit planes until the rotation needs it
     RCHFSI_TRY(gram_i8_full(h, Y, AY, h->B.present ? h->rr2 : nullptr, h->Ha, h->Hb, h->rr3, blk));
     pt.lap("Gram x2 (INT8 tensor pipe, lower)");
   } else {
@@ -185,7 +187,7 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
   const double *E = h->Ha;   // eigenvectors overwrite H_a, column-major
   double *T3 = h->rr3;
   // X = Y E
-  if (rotate_i8_supported(h)) {
+  if (rotate_i8_supported(h) && i8ok) {
     RCHFSI_TRY(rotate_i8(h, Y, m, E, Y, T3, blk));            // in place; T3 holds the digit planes
     pt.lap("X = Y E (INT8 tensor pipe)");
   } else {
@@ -197,17 +199,34 @@ rchfsi_status rayleigh_ritz_impl(rchfsi_ctx *h, double *Y, double *ritz_out, dou
   if (need_res) {
     // AX and BX: either rotate the products already at hand, AX = (AY) E, BX = (BY) E (2 m N^2 flops each), or
     // apply the operators to the rotated block again -- whichever is less work (sparse / FE operators: re-apply)
-    const double *BX = Y;
+    // (rotations on the INT8 pipe run in place -- the products A Y, B Y are dead afterwards -- with the free block as
+    // scratch for the digit planes)
+    const double *AX = T3, *BX = Y;
     const double rot_flops = 2.0 * (double)m * (double)N * (double)N;
-    if (apply_flops(h->A.d, N) < rot_flops) RCHFSI_TRY(apply64(h, h->A.d, Y, T3, N));
-    else RCHFSI_TRY(rotate(h, AY, E, T3));
+    const bool rot8 = rotate_i8_supported(h) && i8ok;
+    if (apply_flops(h->A.d, N) < rot_flops) {
+      RCHFSI_TRY(apply64(h, h->A.d, Y, T3, N));
+    } else if (rot8) {
+      RCHFSI_TRY(rotate_i8(h, AY, m, E, AY, T3, blk));
+      AX = AY;
+    } else {
+      RCHFSI_TRY(rotate(h, AY, E, T3));
+    }
     if (h->B.present) {
-      if (apply_flops(h->B.d, N) < rot_flops) RCHFSI_TRY(apply64(h, h->B.d, Y, h->rr1, N));
-      else RCHFSI_TRY(rotate(h, h->rr2, E, h->rr1));   // AY is dead by then
-      BX = h->rr1;
+      double *spare = (AX == AY) ? T3 : h->rr1;        // the block that holds neither A X nor B Y
+      if (apply_flops(h->B.d, N) < rot_flops) {
+        RCHFSI_TRY(apply64(h, h->B.d, Y, spare, N));
+        BX = spare;
+      } else if (rot8) {
+        RCHFSI_TRY(rotate_i8(h, h->rr2, m, E, h->rr2, spare, blk));
+        BX = h->rr2;
+      } else {
+        RCHFSI_TRY(rotate(h, h->rr2, E, spare));
+        BX = spare;
+      }
     }
     pt.lap("AX, BX (re-apply or rotate)");
-    RCHFSI_TRY(residual_block(h, T3, BX, h->ritz_dev, G_out, res_out, m, N));
+    RCHFSI_TRY(residual_block(h, AX, BX, h->ritz_dev, G_out, res_out, m, N));
     pt.lap("residual block");
   }
   if (ritz_out && ritz_out != h->ritz_dev)
@@ -232,7 +251,8 @@ rchfsi_status rotate_in_place(rchfsi_ctx *h, double *Y, const double *E) {
   }
   choose_row_panel(h);
   if (!h->rrp) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)h->rr_rp * N));
-  if (rotate_i8_supported(h)) return rotate_i8(h, Y, m, E, Y, h->rrp, sizeof(double) * (size_t)h->rr_rp * N);
+  if (rotate_i8_supported(h) && rr_i8_scratch_ok(h, sizeof(double) * (size_t)h->rr_rp * N))
+    return rotate_i8(h, Y, m, E, Y, h->rrp, sizeof(double) * (size_t)h->rr_rp * N);
   const double one = 1.0, zero = 0.0;
   for (int64_t r0 = 0; r0 < m; r0 += h->rr_rp) {
     const int64_t rows = std::min<int64_t>(h->rr_rp, m - r0);
@@ -333,11 +353,12 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
       const uint8_t *p0 = reinterpret_cast<const uint8_t *>(b.ptr);
       if (p0 && !(cells64 && cells64 >= p0 && cells64 < p0 + b.bytes) && b.bytes > rot_bytes) { rot_buf = b.ptr; rot_bytes = b.bytes; }
     }
-  const bool rot8 = rotate_i8_supported(h);
-  if (!(rot8 && rot_buf)) {
+  bool rot8 = rotate_i8_supported(h);
+  if (!(rot8 && rot_buf && rr_i8_scratch_ok(h, rot_bytes))) {
     if (!h->rrp) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrp, sizeof(double) * (size_t)h->rr_rp * N));
     rot_buf = h->rrp;
     rot_bytes = sizeof(double) * (size_t)h->rr_rp * N;
+    rot8 = rot8 && rr_i8_scratch_ok(h, rot_bytes);
   }
   for (int32_t c0 = 0; c0 < N; c0 += cw) {
     const int32_t w = std::min(cw, N - c0);

@@ -723,11 +723,16 @@ __global__ void __launch_bounds__(320, 1) i8w_kernel(const __grid_constant__ I8M
 
 }  // namespace
 
+// scratch the two products need at least (one 128-row chunk of digit planes): tiny problems fall back to dgemm
+bool rr_i8_scratch_ok(const rchfsi_ctx *h, size_t bytes) {
+  const size_t Kp = ((size_t)h->N + 15) / 16 * 16;
+  return bytes >= (size_t)2 * I8_S * h->N * 128 + 8192 && bytes >= ((size_t)I8_S * Kp + 4) * 128 + 4096;
+}
+
 bool rotate_i8_supported(const rchfsi_ctx *h) {
   if (h->knobs.rr_split == 0) return false;
   if (h->N > 16384) return false;                         // INT32 exactness: 7 N 2^14 < 2^31
-  if (h->knobs.rr_split > 0) return h->N >= 16;           // forced (tests at small sizes)
-  return h->N >= 256 && h->m >= 8192;                     // where it beats dgemm
+  return true;   // every size: cuBLAS dgemm stays behind RCHFSI_RR_SPLIT=0 as the reference the tests compare with
 }
 
 size_t rotate_i8_fixed_bytes(int32_t N) {
@@ -819,8 +824,7 @@ rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const dou
 // ---------------------------------------------------------------------------------------- Gram products (host side)
 bool gram_i8_supported(const rchfsi_ctx *h) {
   if (h->knobs.rr_gram_i8 == 0) return false;
-  if (h->knobs.rr_gram_i8 > 0) return h->N >= 16;        // forced (tests at small sizes)
-  return h->N >= 256 && h->m >= 8192;
+  return h->N <= 16384;                                   // every size (RCHFSI_RR_GRAM_I8=0: cuBLAS dgemm, the tests' reference)
 }
 
 bool carve_buf(std::vector<I8Buf> &bufs, size_t bytes, void **out) {
@@ -929,7 +933,7 @@ rchfsi_status gram_finish(rchfsi_ctx *h, int32_t KS, int32_t Nz, int32_t zc0, in
 
 // workspace the INT8 Rayleigh-Ritz products hold beyond the blocks they borrow (planner: automatic choice only)
 size_t rr_i8_plan_bytes(int64_t m, int32_t N) {
-  if (N < 256 || m < 8192 || N > 16384) return 0;
+  if (N > 16384) return 0;
   auto al = [](size_t b) { return (b + 255) / 256 * 256; };
   int64_t tiles = 0;
   for (int a0 = 0; a0 < N; a0 += 128)
