@@ -560,6 +560,9 @@ def bench_c5(args, dev, rank, world, steps, warmup, apply_prec, store_prec):
         sol["certify_seconds"] = time.perf_counter() - t0
         sol["certified"] = bool(sol["converged"] and sol["oracle_residual_max"] <= 1e-8 * 1.01
                                 and sol["oracle_borth_err"] <= 1e-8)
+        # split of the solve's wall time, derived: Alg. 1 runs one Rayleigh-Ritz, then iters x (filter + Rayleigh-Ritz)
+        sol["filter_seconds_each"] = rec["ms_per_step"] * 1e-3
+        sol["rayleigh_ritz_seconds_each_derived"] = max(0.0, sol["seconds"] - sol["iters"] * rec["ms_per_step"] * 1e-3) / (sol["iters"] + 1)
         rec["solve"] = sol
         del X
         torch.cuda.empty_cache()
