@@ -766,7 +766,7 @@ rchfsi_status rotate_i8(rchfsi_ctx *h, const double *In, int64_t rows, const dou
   R = std::min<int64_t>(R, rows);
   if (h->knobs.rr_i8_rows > 0) R = std::min<int64_t>(R, h->knobs.rr_i8_rows);
   if (R >= 128) R = R / 128 * 128;
-  R = std::min<int64_t>(R, 0x7fffff00 / I8_S);
+  R = std::min<int64_t>({R, (int64_t)0x7fffff00 / I8_S, (int64_t)65535 * 128});   // TMA row coordinates, grid.y
   if (R < 1) { h->err = "rotate_i8: scratch too small"; return RCHFSI_EINVAL; }
   int8_t *Aplanes = reinterpret_cast<int8_t *>(scratch);
   int32_t *ea = reinterpret_cast<int32_t *>(Aplanes + ((size_t)I8_S * R * Kp + 255) / 256 * 256);
