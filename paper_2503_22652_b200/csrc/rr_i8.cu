@@ -860,19 +860,24 @@ rchfsi_status colmax(rchfsi_ctx *h, const double *V, int64_t ld, int32_t cols, u
   return RCHFSI_OK;
 }
 
-rchfsi_status slice_t(rchfsi_ctx *h, const double *V, int64_t ld, int64_t r0, int64_t rows, int32_t cols, int64_t Rp,
-                      const unsigned long long *mx, const I8Planes &pl, int32_t *expo) {
-  dim3 grid((unsigned)cdiv(cols, 32), (unsigned)cdiv(rows, 128));
-  i8_slice_t_kernel<<<grid, 256, 0, h->stream>>>(V, ld, r0, rows, cols, Rp, mx, pl, expo);
-  LAUNCH_CHECK(h);
-  return RCHFSI_OK;
-}
-
 I8Planes shifted(const I8Planes &pl, size_t bytes) {
   I8Planes o;
   for (int s = 0; s < I8_S; ++s) o.p[s] = pl.p[s] + bytes;
   return o;
 }
+
+rchfsi_status slice_t(rchfsi_ctx *h, const double *V, int64_t ld, int64_t r0, int64_t rows, int32_t cols, int64_t Rp,
+                      const unsigned long long *mx, const I8Planes &pl, int32_t *expo) {
+  const int64_t span = (int64_t)65535 * 128;             // rows one launch covers (grid.y limit)
+  for (int64_t off = 0; off < rows; off += span) {
+    const int64_t rc = std::min<int64_t>(span, rows - off);
+    dim3 grid((unsigned)cdiv(cols, 32), (unsigned)cdiv(rc, 128));
+    i8_slice_t_kernel<<<grid, 256, 0, h->stream>>>(V, ld, r0 + off, rc, cols, Rp, mx, shifted(pl, (size_t)off), off == 0 ? expo : nullptr);
+    LAUNCH_CHECK(h);
+  }
+  return RCHFSI_OK;
+}
+
 
 int32_t choose_ks(const rchfsi_ctx *h, int32_t N, int32_t Nz, int32_t zc0, bool packed, int64_t rows) {
   const int bn = wide(h) ? I8W_BN : I8_BN;
