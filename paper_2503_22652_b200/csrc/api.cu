@@ -290,7 +290,9 @@ rchfsi_status rchfsi_rayleigh_ritz(rchfsi_handle h, double *Y_in_X_out, double *
     h->err = "rchfsi_rayleigh_ritz: null or misaligned pointer";
     return RCHFSI_EINVAL;
   }
-  if (rr_wants_chunked(h)) return rayleigh_ritz_chunked(h, Y_in_X_out, ritz_out, G_out, RCHFSI_FP64, resnorm_out);
+  const bool chunked = rr_wants_chunked(h);
+  RCHFSI_TRY(rr_preallocate(h, chunked));      // ENOMEM, if any, before the block is touched
+  if (chunked) return rayleigh_ritz_chunked(h, Y_in_X_out, ritz_out, G_out, RCHFSI_FP64, resnorm_out);
   return rayleigh_ritz_impl(h, Y_in_X_out, ritz_out, G_out, resnorm_out);
 }
 

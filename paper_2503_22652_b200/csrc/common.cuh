@@ -322,6 +322,11 @@ size_t fe_lowp_bytes(const rchfsi_operator &A, int prec);
 // scratch of the batched-GEMM FE applies of the Rayleigh-Ritz for an N-column block
 size_t fe_rr_scratch_bytes(const rchfsi_operator &op, int32_t N, int64_t max_cells_per_colour);
 rchfsi_status fe_tc_step(rchfsi_ctx *h, const FusedStep &s);
+// allocate (and build) what the fused step of this plan needs before the first step: rchfsi_solve calls them up front,
+// so that a workspace that is too small shows as ENOMEM before any caller block has been changed
+rchfsi_status csr_fused_prepare(rchfsi_ctx *h, bool chfsi);
+rchfsi_status dense_tc_prepare(rchfsi_ctx *h, int apply_prec, bool chfsi);
+rchfsi_status fe_tc_prepare(rchfsi_ctx *h, int apply_prec, bool chfsi);
 
 // ---- fe_rr.cu / fe_tc.cu ---------------------------------------------------------------
 rchfsi_status fe_build_coloring(rchfsi_ctx *h);    // host side: colours, order, flags; validates conn (create time)
@@ -342,6 +347,9 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
                                     double *res_out);
 bool rr_wants_chunked(rchfsi_ctx *h);
 rchfsi_status rotate_in_place(rchfsi_ctx *h, double *Y, const double *E);   // rchfsi_rotate
+rchfsi_status rr_preallocate(rchfsi_ctx *h, bool chunked);                  // every buffer of a Rayleigh-Ritz, nothing computed
+rchfsi_status fe_rr_preallocate(rchfsi_ctx *h, const rchfsi_operator &op, int32_t N);
+rchfsi_status rr_i8_preallocate(rchfsi_ctx *h, bool chunked, int32_t cw);
 
 // ---- rr_i8.cu: rotation X = Y E on the INT8 tensor pipe (error-free digit split of the FP64 operands) ----
 bool rotate_i8_supported(const rchfsi_ctx *h);

@@ -134,9 +134,9 @@ bool csr_fused_supported(const rchfsi_operator &A, int32_t N, const rchfsi_optio
 }
 size_t csr_lowp_bytes(const rchfsi_operator &A) { return sizeof(float) * (size_t)A.nnz; }
 
-rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s) {
+// the folded FP32 copy of the values: allocated (and built) on first use, or up front by rchfsi_solve
+static rchfsi_status csr_copy(rchfsi_ctx *h, bool folded, LowpCopy **out) {
   const rchfsi_operator &op = h->A.d;
-  const bool folded = !s.chfsi && h->dinv != nullptr;
   LowpCopy *cp = find_copy(h, RCHFSI_FP32, folded);
   if (!cp) {
     LowpCopy c;
@@ -154,6 +154,18 @@ rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s) {
     LAUNCH_CHECK(h);
     cp->stale = false;
   }
+  *out = cp;
+  return RCHFSI_OK;
+}
+rchfsi_status csr_fused_prepare(rchfsi_ctx *h, bool chfsi) {
+  LowpCopy *cp = nullptr;
+  return csr_copy(h, !chfsi && h->dinv != nullptr, &cp);
+}
+
+rchfsi_status csr_fused_step(rchfsi_ctx *h, const FusedStep &s) {
+  const rchfsi_operator &op = h->A.d;
+  LowpCopy *cp = nullptr;
+  RCHFSI_TRY(csr_copy(h, !s.chfsi && h->dinv != nullptr, &cp));
   const double *dinv_out = s.chfsi ? h->dinv : nullptr;
   const dim3 grid((unsigned)cdiv(h->m, CSR_ROWS));
   if (s.store_prec == RCHFSI_FP64)

@@ -487,6 +487,12 @@ void dense_tc_pick(const Knobs &kn, int64_t m, int32_t N, int nkb128, int *bn_ou
   *ks_out = ks;
 }
 
+rchfsi_status dense_tc_prepare(rchfsi_ctx *h, int apply_prec, bool chfsi) {
+  rchfsi_status st;
+  get_dense_copy(h, apply_prec == RCHFSI_BF16 ? RCHFSI_BF16 : RCHFSI_TF32, !chfsi && h->dinv != nullptr, &st);
+  return st;
+}
+
 rchfsi_status dense_tc_step(rchfsi_ctx *h, const FusedStep &s) {
   const bool bf16 = (s.apply_prec == RCHFSI_BF16);
   const bool folded = !s.chfsi && h->dinv != nullptr;

@@ -111,29 +111,19 @@ bool fe_apply_gemm_supported(const rchfsi_ctx *h, const rchfsi_operator &op) {
          op.n_loc == A.n_loc && h->cublas != nullptr && (op.cell_mats != nullptr || op.cell_mats_f32 != nullptr);
 }
 
-rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,
-                            int64_t ldw, int64_t ldt) {
-  if (ldw == 0) ldw = N;
-  if (ldt == 0) ldt = N;
-  RCHFSI_TRY(fe_ensure_coloring(h));
+// scratch of the batched-GEMM apply: gathered operand + product (+ FP64 copy of a batch of FP32 cell matrices when
+// `conv`), about 1.5 GB; sized once for the widest block the handle can see (N_cap or the chunk width of the memory-light
+// Rayleigh-Ritz).  Every buffer has its own guard: a call that ran out of workspace is repeated after the caller added a
+// segment (rchfsi_add_workspace) and must not allocate again what it already has.
+static rchfsi_status feg_ensure(rchfsi_ctx *h, const rchfsi_operator &op, int32_t N, bool conv, int64_t *cap_out) {
   const FeColoring &col = h->coloring;
   const int32_t nl = op.n_loc;
-  // FP64 cell matrices: the caller's, or (FP32-only operators) the copy the Rayleigh-Ritz parked in the filter's dead
-  // blocks for the duration of one call (fe_rr_lend_fp64_cells), or else a per-batch conversion
-  const double *mats64 = op.cell_mats;
-  if (!mats64 && h->feg_A_full && &op == &h->A.d) mats64 = h->feg_A_full;
-  const bool conv = (mats64 == nullptr);
-  const int64_t mper = op.cell_shared ? 0 : (int64_t)nl * nl;
-  // scratch: gathered operand + product (+ FP64 copy of FP32 cell matrices), about 1.5 GB; sized once for the widest
-  // block the handle can see (N_cap or the chunk width of the memory-light Rayleigh-Ritz)
   int64_t max_color = 0;
   for (int k = 0; k < col.n_colors; ++k) max_color = std::max(max_color, col.color_begin[k + 1] - col.color_begin[k]);
   const int32_t Nw = std::max<int32_t>(N, h->feg_N);
   const int64_t cap = fe_rr_cells_per_batch(op, Nw, max_color);
   const size_t need_w = sizeof(double) * (size_t)cap * nl * Nw;
   h->feg_N = Nw;
-  // every buffer has its own guard: a call that ran out of workspace is repeated after the caller added a segment
-  // (rchfsi_add_workspace) and must not allocate again what it already has
   if (h->feg_w_bytes < need_w) {
     if (h->feg_W_bytes < need_w) { RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_W, need_w)); h->feg_W_bytes = need_w; }
     if (h->feg_T_bytes < need_w) { RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_T, need_w)); h->feg_T_bytes = need_w; }
@@ -147,6 +137,32 @@ rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const doub
     RCHFSI_TRY(dev_alloc(h, (void **)&h->feg_ptrs, sizeof(double *) * 3 * (size_t)cap));
     h->feg_ptr_cap = cap;
   }
+  *cap_out = cap;
+  return RCHFSI_OK;
+}
+// the same buffers before the first apply (rchfsi_solve's up-front pass); the per-batch FP64 conversion buffer of an
+// FP32-only operator is left to first use: the Rayleigh-Ritz normally lends a full FP64 copy instead
+rchfsi_status fe_rr_preallocate(rchfsi_ctx *h, const rchfsi_operator &op, int32_t N) {
+  RCHFSI_TRY(fe_ensure_coloring(h));
+  int64_t cap = 0;
+  return feg_ensure(h, op, N, false, &cap);
+}
+
+rchfsi_status fe_apply_gemm(rchfsi_ctx *h, const rchfsi_operator &op, const double *W, double *T, int32_t N,
+                            int64_t ldw, int64_t ldt) {
+  if (ldw == 0) ldw = N;
+  if (ldt == 0) ldt = N;
+  RCHFSI_TRY(fe_ensure_coloring(h));
+  const FeColoring &col = h->coloring;
+  const int32_t nl = op.n_loc;
+  // FP64 cell matrices: the caller's, or (FP32-only operators) the copy the Rayleigh-Ritz parked in the filter's dead
+  // blocks for the duration of one call (fe_rr_lend_fp64_cells), or else a per-batch conversion
+  const double *mats64 = op.cell_mats;
+  if (!mats64 && h->feg_A_full && &op == &h->A.d) mats64 = h->feg_A_full;
+  const bool conv = (mats64 == nullptr);
+  const int64_t mper = op.cell_shared ? 0 : (int64_t)nl * nl;
+  int64_t cap = 0;
+  RCHFSI_TRY(feg_ensure(h, op, N, conv, &cap));
   const int64_t pcap = h->feg_ptr_cap;
   const bool vec2 = (N % 2 == 0) && (ldw % 2 == 0) && (ldt % 2 == 0) && ((reinterpret_cast<uintptr_t>(W) & 15u) == 0) &&
                     ((reinterpret_cast<uintptr_t>(T) & 15u) == 0);

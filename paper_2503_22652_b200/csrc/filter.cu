@@ -381,6 +381,13 @@ rchfsi_status rchfsi_solve(rchfsi_handle h, int32_t method, double *X, int32_t n
     const Plan pl = make_plan(h);
     const bool chf = (method == RCHFSI_METHOD_CHFSI);
     RCHFSI_TRY(ensure_filter_workspace(h, pl, degree, !chf && !g32 && (pl.store != RCHFSI_FP64 || pl.panel)));
+    // ... and everything else a filter or a Rayleigh-Ritz of this solve will allocate (reduced-precision operator
+    // copies, chunk buffers, FE apply scratch, the INT8 products' buffers): nothing is computed on X before the
+    // workspace is known to suffice, so an ENOMEM call can be repeated with X untouched
+    if (pl.fused == 1) RCHFSI_TRY(csr_fused_prepare(h, chf));
+    if (pl.fused == 2) RCHFSI_TRY(dense_tc_prepare(h, h->opt.apply_prec, chf));
+    if (pl.fused == 3) RCHFSI_TRY(fe_tc_prepare(h, h->opt.apply_prec, chf));
+    RCHFSI_TRY(rr_preallocate(h, chunked));
   }
   auto do_rr = [&]() -> rchfsi_status {
     if (chunked) return rayleigh_ritz_chunked(h, X, h->ritz_dev, Gbuf, g32 ? RCHFSI_FP32 : RCHFSI_FP64, h->res_dev);

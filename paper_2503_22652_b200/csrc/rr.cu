@@ -265,25 +265,10 @@ rchfsi_status rotate_in_place(rchfsi_ctx *h, double *Y, const double *E) {
   return RCHFSI_OK;
 }
 
-// ------------------------------------------------------------------------------------------------
-// Chunked variant: no full-size temporary.  Extra device memory: two [m][cw] FP64 chunks and one [rp][N]
-// FP64 row panel (about 6 GB + 3 GB at config 5 instead of 3 x 58.5 GB).
-bool rr_wants_chunked(rchfsi_ctx *h) {
-  if (h->knobs.rr_chunked >= 0) return h->knobs.rr_chunked != 0;               // test / tuning knob
-  if (h->rr_cw > 0) return true;                                               // decided earlier for this handle
-  if (h->rr1) return false;                                                    // full workspace already there
-  size_t free_b = 0, total_b = 0;
-  if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return false;
-  const size_t blk = sizeof(double) * (size_t)h->m * h->N;
-  return free_b < (size_t)(3.3 * (double)blk);
-}
-
-rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, void *G_out, int g_prec,
-                                    double *res_out) {
-  RCHFSI_TRY(ensure_rr_workspace(h, false));
+// chunk width and row panel of the memory-light variant, decided once per handle
+static void choose_chunks(rchfsi_ctx *h) {
   const int64_t m = h->m;
   const int32_t N = h->N;
-  cudaStream_t st = h->stream;
   if (h->rr_cw == 0) {
     // two [m][cw] FP64 chunks: 6 GB, or up to a third of the free memory when there is more (wider chunks make the
     // batched FE applies and the Gram GEMMs more efficient)
@@ -303,6 +288,45 @@ rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, 
     h->rr_cw = (int32_t)cw;
     choose_row_panel(h);
   }
+}
+
+// Every buffer a Rayleigh-Ritz of this handle allocates, without computing anything: rchfsi_solve calls it before its
+// first Rayleigh-Ritz, so that a workspace that is too small shows as ENOMEM before X has been touched.
+rchfsi_status rr_preallocate(rchfsi_ctx *h, bool chunked) {
+  RCHFSI_TRY(ensure_rr_workspace(h, !chunked));
+  int32_t width = h->N;
+  if (chunked) {
+    choose_chunks(h);
+    if (!h->rrc1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)h->m * h->rr_cw));
+    if (!h->rrc2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc2, sizeof(double) * (size_t)h->m * h->rr_cw));
+    width = h->rr_cw;
+  }
+  h->feg_N = std::max(h->feg_N, width);
+  if (fe_apply_gemm_supported(h, h->A.d)) RCHFSI_TRY(fe_rr_preallocate(h, h->A.d, width));
+  if (h->B.present && fe_apply_gemm_supported(h, h->B.d)) RCHFSI_TRY(fe_rr_preallocate(h, h->B.d, width));
+  return rr_i8_preallocate(h, chunked, chunked ? h->rr_cw : h->N);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Chunked variant: no full-size temporary.  Extra device memory: two [m][cw] FP64 chunks and one [rp][N]
+// FP64 row panel (about 6 GB + 3 GB at config 5 instead of 3 x 58.5 GB).
+bool rr_wants_chunked(rchfsi_ctx *h) {
+  if (h->knobs.rr_chunked >= 0) return h->knobs.rr_chunked != 0;               // test / tuning knob
+  if (h->rr_cw > 0) return true;                                               // decided earlier for this handle
+  if (h->rr1) return false;                                                    // full workspace already there
+  size_t free_b = 0, total_b = 0;
+  if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return false;
+  const size_t blk = sizeof(double) * (size_t)h->m * h->N;
+  return free_b < (size_t)(3.3 * (double)blk);
+}
+
+rchfsi_status rayleigh_ritz_chunked(rchfsi_ctx *h, double *Y, double *ritz_out, void *G_out, int g_prec,
+                                    double *res_out) {
+  RCHFSI_TRY(ensure_rr_workspace(h, false));
+  const int64_t m = h->m;
+  const int32_t N = h->N;
+  cudaStream_t st = h->stream;
+  choose_chunks(h);
   // (each buffer has its own guard: the call may be repeated after the caller added workspace)
   if (!h->rrc1) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc1, sizeof(double) * (size_t)m * h->rr_cw));
   if (!h->rrc2) RCHFSI_TRY(dev_alloc(h, (void **)&h->rrc2, sizeof(double) * (size_t)m * h->rr_cw));

@@ -947,6 +947,18 @@ size_t rr_i8_plan_bytes(int64_t m, int32_t N) {
   return al(rotate_i8_fixed_bytes(N)) + al((size_t)N * 36 + 1024) + al(sizeof(double) * (size_t)ks * N * N);
 }
 
+// every buffer the INT8 products of one Rayleigh-Ritz hold themselves (the digit planes live in borrowed blocks)
+rchfsi_status rr_i8_preallocate(rchfsi_ctx *h, bool chunked, int32_t cw) {
+  if (rotate_i8_supported(h) && !h->i8_E) RCHFSI_TRY(dev_alloc(h, &h->i8_E, rotate_i8_fixed_bytes(h->N_cap)));
+  if (gram_i8_supported(h)) {
+    RCHFSI_TRY(i8_fixed(h));
+    const size_t hp = chunked ? sizeof(double) * (size_t)32 * h->N * 2 * cw
+                              : sizeof(double) * (size_t)choose_ks(h, h->N, h->N, 0, false, h->m) * h->N * h->N;
+    RCHFSI_TRY(ensure_hpart(h, hp));
+  }
+  return RCHFSI_OK;
+}
+
 // Full-block variant: H_a = Y^T (AY), H_b = Y^T (BY) (BY == NULL: Y^T Y), lower triangles, column-major.  `scratch`
 // holds the transposed digit planes of one row chunk of Y and of Z.
 rchfsi_status gram_i8_full(rchfsi_ctx *h, const double *Y, const double *AY, const double *BY, double *Ha, double *Hb,
