@@ -68,6 +68,11 @@ def test_config3_full_size_fp64_sampled_columns_and_fused_fp32_path():
     s.filter(P.METHOD_RCHFSI, Xd, torch.as_tensor(ritz).cuda(), torch.as_tensor(G).cuda(), p, *bounds)
     err = np.linalg.norm(Xd.cpu().numpy()[:, cols] - Yo, axis=0) / np.linalg.norm(Yo, axis=0)
     assert err.max() < 1e-4, err
+    # the same call through the host entry point: at this size the block goes through the column-chunked pipeline
+    # (128 + 128 + 44 columns, three streams); columns are independent, so the result is bit for bit the same
+    Xh = torch.as_tensor(X.copy()).pin_memory()
+    s.filter_host(P.METHOD_RCHFSI, Xh, ritz, G, p, *bounds)
+    np.testing.assert_array_equal(Xh.numpy(), Xd.cpu().numpy())
     s.close()
 
 
